@@ -1,0 +1,313 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these compares the oracle with itself: each expected value is a closed
+form typed out here, a value printed in the paper (tests/golden/paper_values.txt),
+an exact identity, or a brute-force computation on a tiny case.
+"Pins" (P1..P12) for the list and what mistake each one catches.
+"""
+import os
+
+import numpy as np
+import pytest
+from scipy import integrate
+
+import workloads as wlmod
+from oracle import negf_dense as od
+from oracle import negf_rgf as orgf
+from oracle import selfenergy as se
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+T = wlmod.T_HOP
+
+
+def _paper_values():
+    vals = {}
+    with open(os.path.join(HERE, "golden", "paper_values.txt")) as fh:
+        for line in fh:
+            line = line.strip()
+            if not line or line.startswith("#"):
+                continue
+            key, val = line.split()[:2]
+            vals[key] = float(val)
+    return vals
+
+
+# ------------------------------------------------------------------ P1: 1D closed form
+
+def test_p1_uniform_chain_surface_gf_closed_form():
+    """north_star: g = (E - sqrt(E^2 - 4t^2))/(2t^2).  Inside the band the retarded
+    value is (E - i sqrt(4t^2 - E^2))/(2t^2); outside it is real and decays like 1/E."""
+    t = 2.5
+    E = np.linspace(-4.9, 4.9, 197)
+    g = se.surface_gf_alternating(E + 1e-13j, t, t)
+    expect = (E - 1j * np.sqrt(4 * t * t - E * E)) / (2 * t * t)
+    assert np.max(np.abs(g - expect)) < 1e-11        # eta = 1e-13 moves g by ~eta/|t| near the edges
+    Eo = np.array([-9.0, -5.5, 5.5, 9.0, 40.0])
+    g = se.surface_gf_alternating(Eo + 0j + 1e-300j, t, t)
+    expect = (Eo - np.sign(Eo) * np.sqrt(Eo * Eo - 4 * t * t)) / (2 * t * t)
+    assert np.max(np.abs(g - expect) / np.abs(expect)) < 1e-13
+
+
+def test_p1_semicircle_ldos_sum_rule():
+    """-Im g/pi is the semicircle sqrt(4t^2-E^2)/(2 pi t^2); it integrates to 1."""
+    t = 2.5
+    val, _ = integrate.quad(
+        lambda E: -se.surface_gf_alternating(np.array([E + 1e-12j]), t, t)[0].imag / np.pi,
+        -2 * t, 2 * t, limit=400)
+    assert abs(val - 1.0) < 1e-8
+
+
+def test_p1_small_z_no_cancellation():
+    """At z -> 0 (t1 = t2) the exact value is g = -i/|t| + z/(2t^2) + O(z^2); the
+    cancelling form loses ~eps/|z|^2 there."""
+    t = 2.5
+    z = np.array([1e-6j, 1e-6 + 1e-6j, -3e-7 + 1e-6j])
+    g = se.surface_gf_alternating(z, t, t)
+    series = -1j / t + z / (2 * t * t) + 1j * z * z / (8 * t ** 3)
+    assert np.max(np.abs(g - series)) < 1e-15
+
+
+# ------------------------------------------------------------------ P2: alternating chain
+
+@pytest.mark.parametrize("t1,t2", [(2.5, 2.5), (4.9, 2.5), (0.46, 2.5), (2.5, 0.46), (1.1, 3.3)])
+def test_p2_alternating_chain_is_fixed_point_and_retarded(t1, t2):
+    """g must satisfy its own continued fraction and have Im g <= 0 (retarded)."""
+    rng = np.random.default_rng(5)
+    z = rng.uniform(-9, 9, 400) + 1j * 10.0 ** rng.uniform(-9, 0.5, 400)
+    g = se.surface_gf_alternating(z, t1, t2)
+    gp = 1.0 / (z - t2 * t2 * g)
+    resid = g - 1.0 / (z - t1 * t1 * gp)
+    assert np.max(np.abs(resid) / np.abs(g)) < 1e-9
+    assert np.all(g.imag <= 1e-18)
+
+
+@pytest.mark.parametrize("t1,t2", [(2.5, 2.5), (4.9, 2.5), (0.46, 2.5)])
+def test_p2_alternating_chain_vs_long_finite_chain(t1, t2):
+    """Brute force: (0,0) element of the Green's function of a 3000-site chain at
+    eta = 0.05 eV (the truncation error decays like exp(-L*eta/|t|))."""
+    L = 3000
+    bonds = np.where(np.arange(L - 1) % 2 == 0, t1, t2)
+    for E in (-6.0, -2.2, -0.3, 0.0, 0.9, 2.6, 5.2):
+        z = E + 0.05j
+        # tridiagonal solve for the first column of (z - H)^-1 by the Thomas recursion from
+        # the far end is itself the continued fraction, so use a dense library solve instead
+        H = np.diag(bonds, 1) + np.diag(bonds, -1)
+        e0 = np.zeros(L, dtype=np.complex128)
+        e0[0] = 1.0
+        col = np.linalg.solve(z * np.eye(L) - H, e0)
+        g = se.surface_gf_alternating(np.array([z]), t1, t2)[0]
+        assert abs(col[0] - g) < 1e-11 * max(1.0, abs(g))
+
+
+def test_p2_sancho_rubio_equals_closed_form_scalar():
+    """Decimation on the 2-site principal layer of an alternating chain (independent
+    algorithm) against the closed form."""
+    t1, t2 = 4.7, 2.5
+    H00 = np.array([[0.0, t1], [t1, 0.0]], dtype=np.complex128)
+    H01 = np.array([[0.0, 0.0], [t2, 0.0]], dtype=np.complex128)
+    z = np.array([-7.3, -2.0, -0.1, 0.0, 0.4, 2.3, 6.9]) + 1e-6j
+    g, iters = se.sancho_rubio(z, H00, H01, tol=1e-12, maxit=200, extra=1)
+    closed = se.surface_gf_alternating(z, t1, t2)
+    assert np.max(np.abs(g[:, 0, 0] - closed)) < 1e-11
+    assert iters.max() < 60
+
+
+def test_p2_sancho_rubio_cnt_lead_fourier_diagonal():
+    """The real-space (17,0) lead is block-circulant: F^dagger g_surf F is diagonal with
+    entries g_alt(z; |b_q|, |t|), b_q = t (1 + exp(2 pi i q / 17))."""
+    n = wlmod.CNT_N
+    ce, co = wlmod.cnt_realspace_couplings()
+    layers = se.block_lead_layers(ce, co, 10, 0.0, 0.0)
+    H00, H01, tau = layers["left"]
+    # (z = 0 exactly is avoided: modes with |b_q| < |t| have a zigzag edge state there,
+    #  g ~ 1/z, and the decimation result is conditioning-limited to ~1e-8 relative.)
+    z = np.array([-0.4, 0.05, 0.2, 0.31, 0.6, 1.3, 3.0]) + 1e-6j
+    g, _ = se.sancho_rubio(z, H00, H01)
+    gs = g[:, :n, :n]
+    F = np.exp(2j * np.pi * np.outer(np.arange(n), np.arange(n)) / n) / np.sqrt(n)
+    gd = F.conj().T @ gs @ F
+    off = gd - np.einsum("kii->ki", gd)[:, :, None] * np.eye(n)
+    assert np.max(np.abs(off)) < 2e-9
+    bq = np.abs(T * (1 + np.exp(2j * np.pi * np.arange(n) / n)))
+    for q in range(n):
+        closed = se.surface_gf_alternating(z, bq[q], abs(T))
+        assert np.max(np.abs(gd[:, q, q] - closed) / np.abs(closed)) < 2e-9
+
+
+# ------------------------------------------------------------------ P3: values printed in the paper
+
+def test_p3_paper_bandgap_and_degeneracy():
+    pv = _paper_values()
+    n = int(pv["cnt_chirality_n"])
+    assert n == wlmod.CNT_N and abs(abs(wlmod.T_HOP) - pv["hopping_abs_eV"]) < 1e-15
+    even, odd = wlmod.cnt_mode_couplings()
+    gaps = 2 * np.abs(np.abs(odd) - np.abs(even))          # gap of subband j of an alternating chain
+    gap = np.sort(gaps.real)
+    assert abs(gap[0] - 0.5426) < 1e-4                     # 2|t| min_q |1 - 2 cos(pi q/17)|
+    assert round(gap[0], 2) == 0.54 and abs(gap[0] - pv["bandgap_eV"]) < 0.01
+    assert abs(gap[0] - gap[1]) < 1e-12                    # doubly degenerate
+    ce, _ = wlmod.cnt_realspace_couplings()
+    ev = np.sort(np.abs(np.linalg.eigvals(ce / T)))
+    assert np.allclose(ev, np.sort(np.abs(2 * np.cos(np.pi * np.arange(n) / n))), atol=1e-12)
+
+
+def test_p3_ring_pitch():
+    """512 rings <-> 54.53 nm = 3/4 a_cc per ring, a_cc = 0.142 nm."""
+    pv = _paper_values()
+    assert abs(pv["rings_N512_length_nm"] / 512 - 0.75 * 0.142) < 2e-4
+
+
+# ------------------------------------------------------------------ P4: integer transmission
+
+def _open_modes(E):
+    even, odd = wlmod.cnt_mode_couplings()
+    b, t = np.abs(even), np.abs(odd)
+    return int(np.sum((np.abs(t - b) < abs(E)) & (abs(E) < t + b)))
+
+
+@pytest.mark.parametrize("kind", ["scalar", "block"])
+def test_p4_integer_transmission_ideal_tube(kind):
+    E = np.array([0.2, 0.3, 0.6, 1.2, 3.0])
+    expect = np.array([_open_modes(e) for e in E])
+    assert list(expect) == [0, 2, 4, 8, 15]
+    w = wlmod.make_config(3 if kind == "block" else 2, N=8, K_neq=8, K_eq=0)
+    w.phi[:] = 0.0
+    w.z_neq = E + 1e-10j
+    w.w_neq = np.ones(len(E))
+    _, Tm = od.charge_and_transmission(w)
+    assert np.max(np.abs(Tm[0] - expect)) < 1e-6
+
+
+def test_p4_uniform_chain_transmission_is_one():
+    w = wlmod.config1(N=12, K_neq=9)
+    w.phi[:] = 0.3
+    w.z_neq = np.linspace(-4.5, 4.5, 9) - 0.3 + 1e-11j
+    _, Tm = od.charge_and_transmission(w)
+    assert np.max(np.abs(Tm[0] - 1.0)) < 1e-7
+    w.z_neq = np.array([-5.4, 5.3]) + 1e-11j
+    w.w_neq = np.ones(2)
+    _, Tm = od.charge_and_transmission(w)
+    assert np.max(np.abs(Tm[0])) < 1e-6
+
+
+# ------------------------------------------------------------------ P5/P6: exact identities
+
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_p5_spectral_identity_and_hermiticity(cfg):
+    """i(G - G^dagger) = G (Gamma_L + Gamma_R + 2 eta I) G^dagger  exactly."""
+    w = wlmod.make_config(cfg, N=10, K_neq=4, K_eq=0)
+    n = w.n
+    eta = 1e-3
+    for E in (-0.35, 0.05, 0.62):
+        if cfg == 2:
+            ce, co = w.coup_even[5:6], w.coup_odd[5:6]
+        else:
+            ce, co = w.coup_even, w.coup_odd
+        G, sL, sR = od.green_dense(-w.phi[0], ce, co, n, E + 1j * eta, w.lead_kind)
+        D = G.shape[0]
+        gam = np.zeros((D, D), dtype=np.complex128)
+        gam[:n, :n] = 1j * (sL - sL.conj().T)
+        gam[D - n:, D - n:] = 1j * (sR - sR.conj().T)
+        lhs = 1j * (G - G.conj().T)
+        rhs = G @ (gam + 2 * eta * np.eye(D)) @ G.conj().T
+        assert np.max(np.abs(lhs - rhs)) < 1e-12 * max(1.0, np.max(np.abs(lhs)))
+        AL = G[:, :n] @ gam[:n, :n] @ G[:, :n].conj().T
+        assert np.max(np.abs(AL - AL.conj().T)) < 1e-13
+        assert np.all(np.diagonal(AL).real > -1e-14)
+        # reciprocity for real H: T_LR = T_RL
+        gL, gR = gam[:n, :n], gam[D - n:, D - n:]
+        TLR = np.trace(gL @ G[:n, D - n:] @ gR @ G[:n, D - n:].conj().T).real
+        TRL = np.trace(gR @ G[D - n:, :n] @ gL @ G[D - n:, :n].conj().T).real
+        assert abs(TLR - TRL) < 1e-12 * max(1.0, abs(TLR))
+
+
+# ------------------------------------------------------------------ P7: real space == sum of modes
+
+def test_p7_real_space_equals_sum_of_modes():
+    wb = wlmod.make_config(3, N=12, K_neq=10, K_eq=6)
+    ws = wlmod.scalar_twin(wb)
+    nb, Tb = od.charge_and_transmission(wb)
+    ns, Ts = od.charge_and_transmission(ws)
+    assert np.max(np.abs(nb - ns) / np.abs(ns)) < 1e-10
+    assert np.max(np.abs(Tb - Ts)) < 1e-9
+
+
+# ------------------------------------------------------------------ P8/P9: energy reduction
+
+def _chain_workload(N, K_neq, K_eq, mu_s, mu_d, kT=wlmod.KT, e_b=-6.0):
+    w = wlmod.config1(N=N, K_neq=8)
+    w.phi[:] = 0.0
+    e_min = min(mu_s, mu_d) - wlmod.F_TAIL * kT
+    e_max = max(mu_s, mu_d) + wlmod.F_TAIL * kT
+    w.z_neq, w.w_neq = wlmod.real_axis_gauss_legendre(e_min, e_max, K_neq)
+    w.z_eq, w.w_eq = wlmod.contour_semicircle(e_b, e_min, K_eq, min(mu_s, mu_d), kT)
+    w.mu_s, w.mu_d, w.kT = mu_s, mu_d, kT
+    return w
+
+
+def test_p8_half_filling():
+    """phi = 0, mu_S = mu_D = 0: exactly 1/2 electron per orbital per spin
+    (bipartite lattice); pins sign, 1/pi vs 1/2pi, deg, contour weights, Fermi factors.
+    Accuracy is eta-limited (the missing 2 eta G G^dagger of P5): ~5e-8."""
+    w = _chain_workload(N=14, K_neq=96, K_eq=48, mu_s=0.0, mu_d=0.0)
+    n, _ = od.charge_and_transmission(w)
+    assert np.max(np.abs(n[0] / w.deg - 0.5)) < 5e-7
+
+
+def test_p9_biased_uniform_chain_density():
+    """Uniform chain under bias: n per spin = int LDOS(E) (f_S + f_D)/2 dE with
+    LDOS = 1/(pi sqrt(4t^2 - E^2)) (bulk site of an infinite chain)."""
+    mu_s, mu_d, kT, t = 0.0, -0.1, 0.0259, 2.5
+
+    def f(E, mu):
+        return 1.0 / (1.0 + np.exp((E - mu) / kT))
+
+    val, _ = integrate.quad(
+        lambda E: (f(E, mu_s) + f(E, mu_d)) / 2 / (np.pi * np.sqrt(4 * t * t - E * E)),
+        -2 * t, 2 * t, points=[mu_d, mu_s], limit=500, epsabs=1e-12, epsrel=1e-12)
+    assert abs(val - 0.4968165483) < 1e-8                   # value quoted in SURVEY P9
+    w = _chain_workload(N=14, K_neq=128, K_eq=48, mu_s=mu_s, mu_d=mu_d)
+    n, _ = od.charge_and_transmission(w)
+    assert np.max(np.abs(n[0] / w.deg - val)) < 5e-7
+
+
+# ------------------------------------------------------------------ P10: brute force, O1 vs O3
+
+def _random_hermitian_device(rng, N, n):
+    ce = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    co = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    U = rng.uniform(-0.5, 0.5, N)
+    return U, ce, co
+
+
+@pytest.mark.parametrize("N,n", [(2, 3), (5, 3), (6, 4), (7, 1), (8, 1)])
+def test_p10_dense_vs_paper_recursion_random_complex_blocks(N, n):
+    """Non-symmetric complex coupling blocks catch beta/gamma and dagger/transpose
+    mistakes; both lead parities (N even / odd) are exercised."""
+    rng = np.random.default_rng(100 + 10 * N + n)
+    U, ce, co = _random_hermitian_device(rng, N, n)
+    if n == 1:
+        ce, co = ce.reshape(1), co.reshape(1)
+    z_neq = rng.uniform(-3, 3, 6) + 1e-3j
+    w_neq = rng.uniform(0.5, 1.5, 6)
+    z_eq = rng.uniform(-3, 3, 4) + 1j * rng.uniform(0.1, 2.0, 4)
+    w_eq = rng.normal(size=4) + 1j * rng.normal(size=4)
+    lead_kind = 0 if n == 1 else 1
+    args = (U, ce, co, n, z_eq, w_eq, z_neq, w_neq, 0.1, -0.2, 0.05, lead_kind)
+    n1, T1 = od.chain_dense(*args)
+    n3, T3 = orgf.chain_charge(*args)
+    assert np.max(np.abs(n1 - n3)) < 1e-11 * np.max(np.abs(n1))
+    assert np.max(np.abs(T1 - T3)) < 1e-11 * max(1.0, np.max(np.abs(T1)))
+
+
+@pytest.mark.parametrize("cfg,kw", [(1, dict(N=30, K_neq=40)),
+                                    (2, dict(N=40, K_neq=24, K_eq=8)),
+                                    (3, dict(N=16, K_neq=12, K_eq=6)),
+                                    (4, dict(C=2, N=14, K_neq=8, K_eq=4))])
+def test_p10_dense_vs_paper_recursion_on_shrunk_configs(cfg, kw):
+    w = wlmod.make_config(cfg, **kw)
+    n1, T1 = od.charge_and_transmission(w)
+    n3, T3 = orgf.charge_and_transmission(w)
+    assert np.max(np.abs(n1 - n3) / np.abs(n1)) < 1e-11
+    tol = 1e-11 * np.maximum(np.abs(T1), 1e-6 * np.max(np.abs(T1)))
+    assert np.all(np.abs(T1 - T3) <= tol + 1e-300)
