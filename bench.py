@@ -1,0 +1,392 @@
+#!/usr/bin/env python
+"""bench.py -- energy-point RGF sweeps per second on one (or N replicated) B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one synthetic
+workload: negf_set_potential -> negf_charge (self-energies, RGF sweeps, energy reduction) ->
+negf_transmission -> the Poisson stand-in (harness code) -> broyden_step on the per-ring
+potential.  The default workload is BASELINE.json configs[1] (zigzag (17,0) tube in mode space:
+17 chains x 1000 rings, 4096 real-axis + 64 contour energies = 70 720 sweeps per step).
+
+One JSON line is printed by rank 0; see DESIGN.md "Measurement" for every key.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "energy-point RGF sweeps/sec (charge+T(E))"
+UNIT = "sweeps/s"
+
+
+# --------------------------------------------------------------------------- helpers
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            d = json.load(fh)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def load_traffic(kernel: str, config: int):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as fh:
+        d = json.load(fh)
+    return d.get(f"{kernel}:config{config}")
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clocks and throttle reasons with NVML during the timed region."""
+
+    def __init__(self, index: int, period: float = 0.05):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def _sample(self):
+        nv = self.nv
+        self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+        r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)) if hasattr(
+            nv, "nvmlDeviceGetCurrentClocksEventReasons") else int(
+            nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+        names = {
+            0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown",
+            0x4: "sw_power_cap", 0x80: "hw_power_brake_slowdown",
+        }
+        for bit, name in names.items():
+            if r & bit:
+                self.reasons.add(name)
+
+    def run(self):
+        if not self.ok:
+            return
+        while not self._stop_evt.is_set():
+            try:
+                self._sample()
+            except Exception:
+                break
+            self._stop_evt.wait(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.ok:
+            try:
+                self._sample()
+            except Exception:
+                pass
+        return {"sm_mhz": (float(np.median(self.samples)) if self.samples else None),
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def dist_setup(n_gpus: int, backend: str = "nccl"):
+    """(rank, world, local_rank); initialises torch.distributed when launched by torchrun."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29500")
+        if not dist.is_initialized():
+            dist.init_process_group(backend=backend, rank=rank, world_size=world)
+    return rank, world, local
+
+
+def dist_barrier(world: int):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+def dist_max_sum(local_ms: float, local_units: float, world: int, device=None):
+    """(max over ranks of local_ms, sum over ranks of local_units).  The path does not shard
+    (replicas only), so this is the only cross-rank traffic."""
+    if world == 1:
+        return local_ms, local_units
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    u = torch.tensor([local_units], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def make_workload(config: int):
+    import workloads
+    wl = workloads.make_config(config)
+    poisson = wl.extra.get("poisson")
+    if poisson is None:
+        rng = np.random.default_rng(wl.seed + 1500)
+        r = rng.uniform(0.5, 1.0, (max(wl.C - 1, 0), wl.N))
+        n0 = wl.deg * (wl.n_modes if wl.kind == "scalar" else wl.n) / 2.0
+        poisson = workloads.PoissonStandIn(kappa=0.2, r=r, n0=n0)
+    return wl, poisson
+
+
+def algorithmic_bytes_per_sweep(wl) -> float:
+    """history bytes per ring-step (one write + one read), times N."""
+    n2 = wl.n * wl.n
+    neq = 32.0 * n2 if wl.kind == "scalar" else 64.0 * n2
+    eq = 32.0 * n2
+    return wl.N * (wl.K_neq * neq + wl.K_eq * eq) / (wl.K_neq + wl.K_eq)
+
+
+def algorithmic_flop_per_sweep(wl) -> float:
+    n3 = wl.n ** 3
+    if wl.kind == "scalar":
+        return wl.N * (wl.K_neq * 50.0 + wl.K_eq * 36.0) / (wl.K_neq + wl.K_eq)
+    return wl.N * (wl.K_neq * 32.0 * n3 + wl.K_eq * 24.0 * n3) / (wl.K_neq + wl.K_eq)
+
+
+# --------------------------------------------------------------------------- reference arm
+
+def cpu_oracle_sample(wl, budget_s: float = 20.0):
+    """Time the oracle (tier O3, as it stands) on a bounded sample of the workload.
+    Returns (sweeps_per_s, cores, sample description, seconds)."""
+    from oracle import negf_rgf
+    U = -wl.phi[0]
+    t0 = time.perf_counter()
+    sweeps = 0
+    if wl.kind == "scalar":
+        modes = 0
+        for j in range(wl.n_modes):
+            negf_rgf.chain_charge(U, wl.coup_even[j:j + 1], wl.coup_odd[j:j + 1], 1, wl.z_eq, wl.w_eq,
+                                  wl.z_neq, wl.w_neq, wl.mu_s, wl.mu_d, wl.kT, 0, chunk=4096)
+            modes += 1
+            sweeps += wl.K_eq + wl.K_neq
+            if time.perf_counter() - t0 > budget_s:
+                break
+        desc = f"channel 0, {modes} of {wl.n_modes} modes x all {wl.K_eq + wl.K_neq} energies"
+    else:
+        chunk, done = 16, 0
+        while done < wl.K_neq and time.perf_counter() - t0 < budget_s:
+            idx = np.arange(done, min(done + chunk, wl.K_neq))
+            sub = wl.subset(neq_idx=idx, eq_idx=[], channels=[0])
+            negf_rgf.charge_and_transmission(sub, chunk=chunk)
+            done += len(idx)
+            sweeps += len(idx)
+        desc = f"channel 0, first {done} real-axis energies of {wl.K_neq}"
+    dt = time.perf_counter() - t0
+    cores = 1   # numpy elementwise / tiny batched LAPACK calls: single-threaded in practice
+    return sweeps / dt, cores, desc, dt
+
+
+def run_reference(args):
+    rank, world, _ = dist_setup(args.gpus, backend="gloo")
+    if rank != 0:
+        return
+    wl, _ = make_workload(args.config)
+    for _ in range(min(args.warmup, 1)):
+        cpu_oracle_sample(wl, budget_s=2.0)
+    tot_sweeps, tot_t, desc = 0.0, 0.0, ""
+    per_step_budget = max(2.0, min(20.0, 90.0 / max(args.steps, 1)))
+    for _ in range(args.steps):
+        sps, cores, desc, dt = cpu_oracle_sample(wl, budget_s=per_step_budget)
+        tot_sweeps += sps * dt
+        tot_t += dt
+    value = tot_sweeps / tot_t
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": f"configs[{args.config - 1}] {wl.name}", "C": wl.C, "N": wl.N,
+                   "block": wl.n, "n_modes": wl.n_modes, "K_neq": wl.K_neq, "K_eq": wl.K_eq},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": desc + " per step (oracle/negf_rgf.py, numpy)"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------- our arm
+
+def run_ours(args):
+    import torch
+    from paper_2407_14633_b200 import Broyden, Negf, negf_fp64_peak
+
+    rank, world, local = dist_setup(args.gpus)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    torch.cuda.set_device(local % torch.cuda.device_count())
+    dev = torch.device("cuda", torch.cuda.current_device())
+
+    wl, poisson = make_workload(args.config)
+    sweeps_per_step = wl.sweeps
+    stream = torch.cuda.current_stream()
+    h = Negf.from_workload(wl, profile=True, stream=stream)
+    bro = Broyden(wl.C * wl.N, history=8, zeta=0.1, stream=stream)
+    phi_ext = torch.tensor(wl.phi, dtype=torch.float64, device=dev)
+    r_dev = torch.tensor(poisson.r, dtype=torch.float64, device=dev)
+    phi = phi_ext.clone()
+    n = torch.empty((wl.C, wl.N), dtype=torch.float64, device=dev)
+    T = torch.empty((wl.C, wl.K_neq), dtype=torch.float64, device=dev)
+
+    def step():
+        h.negf_set_potential(phi)                       # a0 (+ a1b for Sancho-Rubio leads)
+        h.negf_charge(n)                                # a1s, a2, a3, a5
+        h.negf_transmission(T)                          # a4 (cached by negf_charge)
+        phi_out = poisson.phi_out(phi_ext, n, r_dev)    # harness: Poisson stand-in
+        bro.broyden_step(phi.view(-1), phi_out.view(-1), want_eps=False)   # a6
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    h.negf_kernel_stats(reset=True)
+    dist_barrier(world)
+    sampler = ClockSampler(torch.cuda.current_device())
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    dist_barrier(world)
+    clocks = sampler.stop()
+    local_ms = e0.elapsed_time(e1)
+    stats = h.negf_kernel_stats(reset=True)
+    n_final = n.cpu().numpy()
+    assert np.all(np.isfinite(n_final)), "non-finite charge in the timed loop"
+
+    # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
+    phi_host = torch.tensor(wl.phi, dtype=torch.float64).pin_memory()
+    n_host = torch.empty((wl.C, wl.N), dtype=torch.float64).pin_memory()
+    T_host = torch.empty((wl.C, wl.K_neq), dtype=torch.float64).pin_memory()
+    for _ in range(max(1, min(args.warmup, 3))):
+        h.negf_solve_host(phi_host, n_host, T_host)
+    dist_barrier(world)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2.record(stream)
+    for _ in range(args.steps):
+        h.negf_solve_host(phi_host, n_host, T_host)
+    e3.record(stream)
+    torch.cuda.synchronize()
+    e2e_wall_ms = (time.perf_counter() - t0) * 1e3
+    e2e_local_ms = max(e2.elapsed_time(e3), e2e_wall_ms)   # host-synchronous call: wall clock bounds it
+    dist_barrier(world)
+    h.negf_kernel_stats(reset=True)
+
+    ms, units = dist_max_sum(local_ms, float(sweeps_per_step * args.steps), world, dev)
+    e2e_ms, e2e_units = dist_max_sum(e2e_local_ms, float(sweeps_per_step * args.steps), world, dev)
+    if rank != 0:
+        return
+
+    # ---- roofline of the dominant kernel
+    kname = "scalar_sweep" if wl.kind == "scalar" else "block_sweep"
+    launches, k_ms = stats.get(kname, (0, 0.0))
+    per_launch_ms = k_ms / max(launches, 1)
+    launches_per_step = max(launches, 1) / args.steps
+    hbm_peak, peak_src = load_peaks()
+    if wl.kind == "scalar":
+        alg_bytes = algorithmic_bytes_per_sweep(wl) * sweeps_per_step / launches_per_step
+        achieved = alg_bytes / (per_launch_ms * 1e-3) / 1e9 if per_launch_ms > 0 else 0.0
+        roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
+                    "frac": achieved / hbm_peak, "traffic": load_traffic(kname, args.config),
+                    "kernel": kname, "kernel_ms_per_launch": per_launch_ms,
+                    "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src}
+    else:
+        dfma, dmma = negf_fp64_peak()
+        alg_flop = algorithmic_flop_per_sweep(wl) * sweeps_per_step / launches_per_step
+        achieved = alg_flop / (per_launch_ms * 1e-3) / 1e12 if per_launch_ms > 0 else 0.0
+        roofline = {"bound": "alu", "achieved": achieved, "peak": dfma, "unit": "TFLOP/s",
+                    "frac": achieved / dfma if dfma > 0 else None,
+                    "traffic": load_traffic(kname, args.config), "kernel": kname,
+                    "kernel_ms_per_launch": per_launch_ms, "algorithmic_flop_per_launch": alg_flop,
+                    "peak_source": "FP64 DFMA chain measured live (negf_fp64_peak); DMMA: %.1f" % dmma}
+    kernel_share = {k: round(v[1] / ms, 4) for k, v in stats.items() if v[0]}
+
+    cpu_baseline = None
+    if world == 1:
+        cpu_sps, cores, desc, cpu_dt = cpu_oracle_sample(wl, budget_s=args.cpu_budget)
+        cpu_baseline = {"value": cpu_sps, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": desc + f" ({cpu_dt:.1f} s, oracle/negf_rgf.py)"}
+
+    # my kernels per step: negate + sweep batches + 2-level row reduce + mode reduce + Broyden
+    plan = h.negf_get_plan()
+    my_launches = args.steps * (1 + plan["n_batches"] + 3 + 4)
+    value = units / (ms * 1e-3)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"configs[{args.config - 1}] {wl.name}", "C": wl.C, "N": wl.N,
+                   "block": wl.n, "n_modes": wl.n_modes, "K_neq": wl.K_neq, "K_eq": wl.K_eq,
+                   "sweeps_per_step": sweeps_per_step, "parallelism": f"replicas x{world}",
+                   "l2": "recursion history %.2f GB per step >> 126 MB L2 (no flush needed)" % (
+                       plan["history_bytes"] / 1e9),
+                   "step": "set_potential+charge+transmission+poisson_stand_in+broyden_step"},
+        "clocks": clocks,
+        "e2e": {"value": e2e_units / (e2e_ms * 1e-3), "unit": UNIT,
+                "h2d_bytes_per_step": int(phi_host.numel() * 8),
+                "d2h_bytes_per_step": int((n_host.numel() + T_host.numel()) * 8),
+                "ms_per_step": e2e_ms / args.steps, "call": "negf_solve_host (pinned host buffers)"},
+        "gpu_launches": int(my_launches),
+        "roofline": roofline,
+        "kernel_share_of_step": kernel_share,
+        "cpu_baseline": cpu_baseline,
+    }
+    print(json.dumps(line), flush=True)
+    h.negf_destroy()
+    bro.broyden_destroy()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config, 1-based")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-budget", type=float, default=15.0, dest="cpu_budget")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3            # timing rule: W >= 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+    try:
+        import torch.distributed as dist
+        if dist.is_initialized():
+            dist.destroy_process_group()
+    except Exception:
+        pass
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,140 @@
+"""GPU parity, scalar (mode-space) path: configs[0] and configs[1] of BASELINE.json through the
+C-ABI against the CPU oracle, element by element (north_star: 1e-10 relative)."""
+import numpy as np
+import pytest
+
+import workloads as wlmod
+from oracle import negf_dense as od
+from oracle import negf_rgf as orgf
+from tests.parity import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+
+def _gpu_run(wl, **kw):
+    import torch
+    from paper_2407_14633_b200 import Negf
+    h = Negf.from_workload(wl, **kw)
+    phi = torch.tensor(wl.phi, dtype=torch.float64, device="cuda")
+    n = torch.empty((wl.C, wl.N), dtype=torch.float64, device="cuda")
+    T = torch.empty((wl.C, max(wl.K_neq, 1)), dtype=torch.float64, device="cuda")
+    h.negf_set_potential(phi)
+    h.negf_charge(n)
+    h.negf_transmission(T)
+    h.negf_sync()
+    out = n.cpu().numpy(), T.cpu().numpy()[:, :wl.K_neq]
+    h.negf_destroy()
+    return out
+
+
+def test_config1_full_vs_dense_definition():
+    wl = wlmod.config1()
+    n_ref, T_ref = od.charge_and_transmission(wl)
+    n, T = _gpu_run(wl)
+    assert_parity(n, n_ref, "config1 charge")
+    assert_parity(T, T_ref, "config1 T(E)")
+
+
+@pytest.mark.parametrize("N,K_neq,K_eq", [(40, 37, 9), (33, 64, 16), (2, 5, 3), (17, 1, 0), (50, 0, 7)])
+def test_config2_shrunk_vs_dense_definition(N, K_neq, K_eq):
+    """Several tiles (N > 16) and ragged tails (N % 16 != 0, K % 32 != 0), both lead parities,
+    the degenerate N = 2, contour-only and real-axis-only handles."""
+    wl = wlmod.make_config(2, N=N, K_neq=max(K_neq, 1), K_eq=K_eq)
+    if K_neq == 0:
+        wl = wl.subset(neq_idx=[])
+    n_ref, T_ref = od.charge_and_transmission(wl)
+    n, T = _gpu_run(wl)
+    assert_parity(n, n_ref, "config2-shrunk charge")
+    if K_neq:
+        assert_parity(T, T_ref, "config2-shrunk T(E)")
+
+
+def test_config2_full_vs_paper_recursion():
+    """Full configs[1] (the bench workload, same launch configuration) against tier O3."""
+    wl = wlmod.config2()
+    n_ref, T_ref = orgf.charge_and_transmission(wl)
+    n, T = _gpu_run(wl)
+    assert_parity(n, n_ref, "config2 charge")
+    assert_parity(T, T_ref, "config2 T(E)")
+
+
+def test_config2_full_sampled_vs_dense_definition():
+    """Sampled energies of the full-size device against the dense definition (tier O1)."""
+    wl = wlmod.config2()
+    rng = np.random.default_rng(7)
+    sub = wl.subset(neq_idx=np.sort(rng.choice(wl.K_neq, 3, replace=False)),
+                    eq_idx=np.sort(rng.choice(wl.K_eq, 2, replace=False)))
+    n_ref, T_ref = od.charge_and_transmission(sub)
+    n, T = _gpu_run(sub)
+    assert_parity(n, n_ref, "config2 sampled charge")
+    assert_parity(T, T_ref, "config2 sampled T(E)")
+
+
+def test_workspace_tiling_gives_identical_results():
+    """A small workspace cap forces several sweep launches; results must not change."""
+    wl = wlmod.make_config(2, N=64, K_neq=96, K_eq=16)
+    n1, T1 = _gpu_run(wl)
+    n2, T2 = _gpu_run(wl, workspace_bytes=64 * 32 * 16 * 5)
+    assert np.array_equal(n1, n2) and np.array_equal(T1, T2)
+
+
+def test_multi_channel_scalar_and_host_path():
+    import torch
+    from paper_2407_14633_b200 import Negf
+    wl = wlmod.make_config(2, N=48, K_neq=40, K_eq=8)
+    rng = np.random.default_rng(3)
+    wl.C = 3
+    wl.phi = np.stack([wl.phi[0], wl.phi[0] + 0.05 * rng.normal(size=wl.N), -wl.phi[0]])
+    n_ref, T_ref = od.charge_and_transmission(wl)
+    n, T = _gpu_run(wl)
+    assert_parity(n, n_ref, "3-channel charge")
+    assert_parity(T, T_ref, "3-channel T(E)")
+    h = Negf.from_workload(wl)
+    n_host = np.empty((wl.C, wl.N))
+    T_host = np.empty((wl.C, wl.K_neq))
+    h.negf_solve_host(np.ascontiguousarray(wl.phi), n_host, T_host)
+    assert np.array_equal(n_host, n) and np.array_equal(T_host, T)
+    h.negf_destroy()
+
+
+def test_state_errors_and_rerun():
+    import torch
+    from paper_2407_14633_b200 import Negf, NegfError
+    wl = wlmod.make_config(2, N=20, K_neq=8, K_eq=4)
+    h = Negf.from_workload(wl)
+    n = torch.empty((1, wl.N), dtype=torch.float64, device="cuda")
+    with pytest.raises(NegfError) as ei:
+        h.negf_charge(n)
+    assert ei.value.status == 5                      # NEGF_ESTATE
+    phi = torch.tensor(wl.phi, dtype=torch.float64, device="cuda")
+    h.negf_set_potential(phi)
+    h.negf_charge(n)
+    a = n.cpu().numpy().copy()
+    h.negf_set_potential(phi * 0.5)
+    h.negf_charge(n)
+    b = n.cpu().numpy().copy()
+    h.negf_set_potential(phi)
+    h.negf_charge(n)
+    assert np.array_equal(a, n.cpu().numpy()) and not np.array_equal(a, b)   # deterministic
+    h.negf_destroy()
+
+
+def test_landauer_reductions():
+    """eq.(5)-(6): current and zero-bias conductance from T(E); ideal tube at low kT gives
+    G = G_0 * (number of open modes)."""
+    import torch
+    from paper_2407_14633_b200 import Negf
+    wl = wlmod.make_config(2, N=24, K_neq=64, K_eq=0)
+    wl.phi[:] = 0.0
+    wl.mu_s = wl.mu_d = 0.6
+    wl.kT = 0.002
+    wl.z_neq, wl.w_neq = wlmod.real_axis_gauss_legendre(0.6 - 0.05, 0.6 + 0.05, 64, eta=1e-9)
+    h = Negf.from_workload(wl)
+    h.negf_set_potential(torch.tensor(wl.phi, dtype=torch.float64, device="cuda"))
+    cur = torch.empty(1, dtype=torch.float64, device="cuda")
+    cond = torch.empty(1, dtype=torch.float64, device="cuda")
+    h.negf_current(cur, cond)
+    h.negf_sync()
+    assert abs(cond.item() - 4.0) < 1e-4             # 4 open subbands at E = 0.6 eV
+    assert abs(cur.item()) < 1e-12                   # mu_s == mu_d
+    h.negf_destroy()
