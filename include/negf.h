@@ -159,6 +159,12 @@ NEGF_API negf_status broyden_destroy(broyden_handle* h);
  * of the FP64-bound block kernels.  Synchronous; takes a few milliseconds. */
 NEGF_API negf_status negf_fp64_peak(double* dfma_tflops, double* dmma_tflops);
 
+/* Diagnostic / test hook of the block path's in-register Gauss-Jordan inversion: a diagonal pivot
+ * candidate is accepted when |a_kk| >= theta * max_j |a_kj|, otherwise the task searches the whole
+ * column (partial pivoting).  theta <= 0 restores the default (1e-3); a huge theta (e.g. 1e150) forces
+ * the search at every elimination step.  Process-wide; affects kernels launched afterwards. */
+NEGF_API negf_status negf_set_pivot_threshold(double theta);
+
 /* Last error text of the calling thread (static storage, never NULL). */
 NEGF_API const char* negf_last_error(void);
 /* Library version string, e.g. "negf_b200 0.1 (sm_100a)". */

@@ -27,7 +27,7 @@ EXPORTED_SYMBOLS = [
     "negf_create", "negf_destroy", "negf_set_potential", "negf_charge", "negf_transmission",
     "negf_current", "negf_solve_host", "negf_sync", "negf_kernel_stats", "negf_get_plan",
     "broyden_create", "broyden_step", "broyden_reset", "broyden_destroy",
-    "negf_fp64_peak", "negf_last_error", "negf_version",
+    "negf_fp64_peak", "negf_set_pivot_threshold", "negf_last_error", "negf_version",
 ]
 
 
@@ -95,6 +95,7 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
         "broyden_reset": (C.c_int, [vp]),
         "broyden_destroy": (C.c_int, [vp]),
         "negf_fp64_peak": (C.c_int, [C.POINTER(dbl), C.POINTER(dbl)]),
+        "negf_set_pivot_threshold": (C.c_int, [dbl]),
         "negf_last_error": (C.c_char_p, []),
         "negf_version": (C.c_char_p, []),
     }
@@ -293,6 +294,10 @@ def negf_fp64_peak():
     a, b = C.c_double(0.0), C.c_double(0.0)
     _check(load_library().negf_fp64_peak(C.byref(a), C.byref(b)), "negf_fp64_peak")
     return a.value, b.value
+
+
+def negf_set_pivot_threshold(theta: float) -> None:
+    _check(load_library().negf_set_pivot_threshold(float(theta)), "negf_set_pivot_threshold")
 
 
 def negf_version() -> str:

@@ -1,0 +1,275 @@
+// Device primitives of the block (n x n, real-space) path: thread geometry, shared-memory layout,
+// in-register Gauss-Jordan inversion, sparse coupling products and block reductions.
+//
+// Geometry: one thread owns one ROW of its task's n x n complex matrix
+// in registers; n consecutive threads form a task (one (channel, energy, direction) recursion);
+// TPC tasks share a CTA and advance ring by ring in lock step.  Tasks straddle warp boundaries
+// (17 does not divide 32), so rows are exchanged through shared memory and CTA barriers, never
+// through shuffles.  With n = 17: 15 tasks = 255 live threads + 1 ghost thread per 256-thread CTA.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace negf {
+namespace blk {
+
+typedef double2 c64;
+
+__device__ __forceinline__ c64 cmul(c64 a, c64 b) {
+  return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ c64 cconj(c64 a) { return make_double2(a.x, -a.y); }
+// acc += a * b
+__device__ __forceinline__ void cfma(c64& acc, c64 a, c64 b) {
+  acc.x = fma(a.x, b.x, acc.x);
+  acc.x = fma(-a.y, b.y, acc.x);
+  acc.y = fma(a.x, b.y, acc.y);
+  acc.y = fma(a.y, b.x, acc.y);
+}
+// acc -= a * b
+__device__ __forceinline__ void cfms(c64& acc, c64 a, c64 b) {
+  acc.x = fma(-a.x, b.x, acc.x);
+  acc.x = fma(a.y, b.y, acc.x);
+  acc.y = fma(-a.x, b.y, acc.y);
+  acc.y = fma(-a.y, b.x, acc.y);
+}
+__device__ __forceinline__ double cabs2(c64 a) { return fma(a.x, a.x, a.y * a.y); }
+__device__ __forceinline__ c64 crcp(c64 d) {
+  const double r = 1.0 / cabs2(d);
+  return make_double2(d.x * r, -d.y * r);
+}
+
+template <int NB>
+struct Geo {
+  static constexpr int TPC = (255 / NB) > 32 ? 32 : (255 / NB);   // tasks per CTA
+  static constexpr int LIVE = TPC * NB;                            // threads that own a row
+  static constexpr int THREADS = (LIVE + 31) / 32 * 32;            // CTA size (ghosts pad the last warp)
+  static constexpr int NWARPS = THREADS / 32;
+  static constexpr int MAT = NB * NB;
+  // one ring step of recursion history of one CTA: [column b][thread] complex, 16-byte coalesced
+  static constexpr int64_t STEP_ELEMS = (int64_t)NB * THREADS;
+};
+
+// Sparse matrix in CSR form, read-only in shared memory.
+struct Csr {
+  const int* rowptr;   // [NB + 1]
+  const int* col;      // [nnz]
+  const c64* val;      // [nnz]
+};
+
+// Shared-memory working set of one CTA (carved from dynamic shared memory).
+template <int NB>
+struct Smem {
+  c64* mat;      // [TPC][NB*NB]   one exchange matrix per task
+  c64* prow;     // [2][TPC][NB]   published pivot rows (double buffered by elimination step)
+  double* mag;   // [TPC][NB]      pivot-search magnitudes / small per-task reductions
+  int* pk;       // [2][TPC]       pivot row of the current elimination step
+  int* perm;     // [TPC][NB]      pivot row chosen for column k
+  int* ok;       // [TPC]          1 if the diagonal candidate was accepted this step
+  double* red;   // [2][NWARPS]    block reduction scratch
+
+  static constexpr size_t bytes(int nmat = 1) {
+    using G = Geo<NB>;
+    return sizeof(c64) * ((size_t)nmat * G::TPC * G::MAT + 2 * G::TPC * NB) +
+           sizeof(double) * (G::TPC * NB + 2 * G::NWARPS) + sizeof(int) * (2 * G::TPC + G::TPC * NB + G::TPC) + 64;
+  }
+  // returns the first byte after the carved region (16-byte aligned)
+  __device__ char* carve(char* base, int nmat = 1) {
+    using G = Geo<NB>;
+    mat = reinterpret_cast<c64*>(base);
+    prow = mat + (size_t)nmat * G::TPC * G::MAT;
+    mag = reinterpret_cast<double*>(prow + 2 * G::TPC * NB);
+    red = mag + G::TPC * NB;
+    pk = reinterpret_cast<int*>(red + 2 * G::NWARPS);
+    perm = pk + 2 * G::TPC;
+    ok = perm + G::TPC * NB;
+    char* end = reinterpret_cast<char*>(ok + G::TPC);
+    return reinterpret_cast<char*>((reinterpret_cast<uintptr_t>(end) + 15) & ~uintptr_t(15));
+  }
+};
+
+// Default threshold of the diagonal-candidate test in gj_invert: the candidate pivot is accepted
+// when |a_kk|^2 >= theta2 * max_j |a_kj|^2 (normalised pivot-row entries bounded by 1/theta = 1e3);
+// otherwise the task falls back to a full column search over its unused rows.
+constexpr double kTheta2Default = 1e-6;
+
+// In-place Gauss-Jordan inversion of the task's matrix, rows in registers (r = row `a`).
+// Pivoting is implicit (rows never move): on return, thread i holds row q(i) of the inverse with
+// column j of its registers being inverse column perm[j], where perm[k] is the pivot row chosen for
+// column k and q = perm^-1.  Returns (CTA-uniform) whether any task left the diagonal pivot order; if
+// not, perm is the identity and r is row a of the inverse as is.
+// Barriers: one __syncthreads_or per elimination step (+2 on the rare search path).  The caller
+// must place at least one CTA barrier between two consecutive calls.
+template <int NB>
+__device__ __forceinline__ bool gj_invert(c64 (&r)[NB], const Smem<NB>& sm, int t, int a, bool live,
+                                          double theta2) {
+  using G = Geo<NB>;
+  bool used = false;
+  bool any_search = false;
+#pragma unroll
+  for (int k = 0; k < NB; ++k) {
+    const int buf = k & 1;
+    c64* prow = sm.prow + ((size_t)buf * G::TPC + t) * NB;
+    int bad = 0;
+    if (a == k) {
+      bool accept = false;
+      if (!used) {
+        const double m = cabs2(r[k]);
+        double rm = 0.0;
+#pragma unroll
+        for (int j = 0; j < NB; ++j)
+          if (j != k) rm = fmax(rm, cabs2(r[j]));
+        accept = (m >= theta2 * rm) && (m > 0.0);
+      }
+      if (accept) {
+        const c64 inv = crcp(r[k]);
+#pragma unroll
+        for (int j = 0; j < NB; ++j) r[j] = (j == k) ? inv : cmul(r[j], inv);
+        used = true;
+        if (live) {
+#pragma unroll
+          for (int j = 0; j < NB; ++j) prow[j] = r[j];
+          sm.pk[buf * G::TPC + t] = a;
+          sm.perm[t * NB + k] = a;
+        }
+      }
+      if (live) sm.ok[t] = accept ? 1 : 0;
+      bad = (live && !accept) ? 1 : 0;
+    }
+    if (__syncthreads_or(bad)) {
+      // rare path: every task whose candidate was rejected searches column k over its unused rows
+      any_search = true;
+      const bool need = sm.ok[t] == 0;
+      if (need && live) sm.mag[t * NB + a] = used ? -1.0 : cabs2(r[k]);
+      __syncthreads();
+      if (need) {
+        int best = 0;
+        double bm = sm.mag[t * NB];
+#pragma unroll
+        for (int i = 1; i < NB; ++i) {
+          const double v = sm.mag[t * NB + i];
+          if (v > bm) { bm = v; best = i; }
+        }
+        if (a == best) {
+          const c64 inv = crcp(r[k]);
+#pragma unroll
+          for (int j = 0; j < NB; ++j) r[j] = (j == k) ? inv : cmul(r[j], inv);
+          used = true;
+          if (live) {
+#pragma unroll
+            for (int j = 0; j < NB; ++j) prow[j] = r[j];
+            sm.pk[buf * G::TPC + t] = a;
+            sm.perm[t * NB + k] = a;
+          }
+        }
+      }
+      __syncthreads();
+    }
+    const int p = sm.pk[buf * G::TPC + t];
+    if (a != p) {
+      const c64 f = r[k];
+      r[k] = make_double2(0.0, 0.0);
+#pragma unroll
+      for (int j = 0; j < NB; ++j) cfms(r[j], f, prow[j]);
+    }
+  }
+  return any_search;
+}
+
+// Write the inverse left in registers by gj_invert to the task's exchange matrix in logical
+// (row, column) order.  Needs a barrier before anyone reads other rows.
+template <int NB>
+__device__ __forceinline__ void store_inverse(const c64 (&r)[NB], c64* mat_t, const Smem<NB>& sm, int t,
+                                              int a, bool live, bool permuted) {
+  if (!live) return;
+  if (!permuted) {
+#pragma unroll
+    for (int j = 0; j < NB; ++j) mat_t[a * NB + j] = r[j];
+  } else {
+    const int* perm = sm.perm + t * NB;
+    int row = 0;
+#pragma unroll
+    for (int k = 0; k < NB; ++k)
+      if (perm[k] == a) row = k;
+#pragma unroll
+    for (int j = 0; j < NB; ++j) mat_t[row * NB + perm[j]] = r[j];
+  }
+}
+
+// y[b] = sum_{c in nz(K_a)} K[a][c] * X[c][b]      (row a of K X, X in shared memory)
+template <int NB>
+__device__ __forceinline__ void sparse_left(c64 (&y)[NB], const Csr& K, const c64* X, int a) {
+#pragma unroll
+  for (int b = 0; b < NB; ++b) y[b] = make_double2(0.0, 0.0);
+  const int e1 = K.rowptr[a + 1];
+  for (int e = K.rowptr[a]; e < e1; ++e) {
+    const c64 v = K.val[e];
+    const c64* xr = X + K.col[e] * NB;
+#pragma unroll
+    for (int b = 0; b < NB; ++b) cfma(y[b], v, xr[b]);
+  }
+}
+
+// y[b] = sum_{d in nz(K_b)} xrow[d] * conj(K[b][d])   (row of X K^dagger, xrow = this thread's row in
+// shared memory)
+template <int NB>
+__device__ __forceinline__ void sparse_right_dagger(c64 (&y)[NB], const Csr& K, const c64* xrow) {
+#pragma unroll
+  for (int b = 0; b < NB; ++b) {
+    c64 acc = make_double2(0.0, 0.0);
+    const int e1 = K.rowptr[b + 1];
+    for (int e = K.rowptr[b]; e < e1; ++e) cfma(acc, xrow[K.col[e]], cconj(K.val[e]));
+    y[b] = acc;
+  }
+}
+
+// c[b] = sum_k arow[k] * X[k][b]   (row of A X: A row in registers, X in shared memory)
+template <int NB>
+__device__ __forceinline__ void gemm_row(c64 (&c)[NB], const c64 (&arow)[NB], const c64* X) {
+#pragma unroll
+  for (int b = 0; b < NB; ++b) c[b] = make_double2(0.0, 0.0);
+#pragma unroll
+  for (int k = 0; k < NB; ++k) {
+    const c64 av = arow[k];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) cfma(c[b], av, X[k * NB + b]);
+  }
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+__device__ __forceinline__ double fermi(double E, double mu, double kT) {
+  const double x = (E - mu) / kT;
+  const double e = exp(-fabs(x));
+  return x > 0.0 ? e / (1.0 + e) : 1.0 / (1.0 + e);
+}
+
+// Copy a CSR matrix from global to shared memory (all threads; caller barriers afterwards).
+__device__ __forceinline__ char* csr_to_shared(Csr& dst, char* base, const int* g_rowptr, const int* g_col,
+                                               const c64* g_val, int nb, int nnz_cap) {
+  // layout: val[nnz_cap] (16-byte aligned), rowptr[nb+1], col[nnz_cap]
+  c64* val = reinterpret_cast<c64*>(base);
+  int* rowptr = reinterpret_cast<int*>(val + nnz_cap);
+  int* col = rowptr + nb + 1;
+  const int nnz = g_rowptr[nb];
+  for (int i = threadIdx.x; i <= nb; i += blockDim.x) rowptr[i] = g_rowptr[i];
+  for (int i = threadIdx.x; i < nnz; i += blockDim.x) {
+    col[i] = g_col[i];
+    val[i] = g_val[i];
+  }
+  dst.rowptr = rowptr;
+  dst.col = col;
+  dst.val = val;
+  char* end = reinterpret_cast<char*>(col + nnz_cap);
+  return reinterpret_cast<char*>((reinterpret_cast<uintptr_t>(end) + 15) & ~uintptr_t(15));
+}
+__host__ __device__ constexpr size_t csr_shared_bytes(int nb, int nnz_cap) {
+  return ((sizeof(double2) * (size_t)nnz_cap + sizeof(int) * (size_t)(nb + 1 + nnz_cap)) + 15) / 16 * 16;
+}
+
+}  // namespace blk
+}  // namespace negf

@@ -1,18 +1,300 @@
-// Placeholder until the block kernels land: fails loudly (no CPU fallback, no silent success).
+// Host side of the block (real-space, n x n) path: coupling tables, workspace plan, launch
+// sequencing of sancho_rubio.cu / block_sweep.cu / reduce.cu.  No arithmetic of the method runs
+// here except the constant n x n products of the coupling blocks that define the lead's reduced
+// chain (sancho_rubio.cu header), computed once at creation.
+#include <algorithm>
+#include <complex>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "block_ops.cuh"
 #include "block_path.h"
 #include "negf_internal.h"
 
 namespace negf {
-struct BlockPath { int dummy; };
-negf_status block_path_create(const negf_config*, const double2*, const double2*, const double2*,
-                              const double*, BlockPath** out) {
-  *out = nullptr;
-  set_error("block > 1 path is not built in this version of libnegf_b200");
-  return NEGF_EINVAL;
+
+using blk::CsrSet;
+typedef std::complex<double> zc;
+
+struct BlockPath {
+  int C, N, n, K_eq, K_neq;
+  double mu_s, mu_d, kT, deg, sr_tol;
+  int sr_maxit;
+  const double2 *z_eq, *w_eq, *z_neq;   // owned by the negf_handle
+  const double* w_neq;
+  // geometry
+  int tpc, threads, geq, gneq;
+  long long total_cta, n_eq_cta;
+  int slots, wave, ctas_per_sm, n_launches;
+  int64_t slot_bytes, hist_bytes, partial_bytes, table_bytes;
+  // device
+  int* csr_rowptr;
+  int* csr_col;
+  double2* csr_val;
+  int nnz_cap;
+  double2* lead_mats;
+  double2* table;
+  double2* hist;
+  double* partial;
+  double* scratch;
+  int* flags;       // [0] max SR iterations, [1] non-convergence flag
+  int last_max_iters;
+};
+
+static double g_theta2 = blk::kTheta2Default;
+void block_path_set_pivot_threshold(double theta) {
+  g_theta2 = theta > 0.0 ? theta * theta : blk::kTheta2Default;
 }
-negf_status block_path_self_energy(BlockPath*, const double*, cudaStream_t, ProfHook) { return NEGF_EINVAL; }
-negf_status block_path_run(BlockPath*, const double*, double*, double*, cudaStream_t, ProfHook) { return NEGF_EINVAL; }
-negf_status block_path_check(BlockPath*) { return NEGF_OK; }
-void block_path_plan(BlockPath*, negf_plan_info*) {}
-void block_path_destroy(BlockPath*) {}
+
+namespace {
+
+std::vector<zc> mat_mul(const std::vector<zc>& A, const std::vector<zc>& B, int n) {
+  std::vector<zc> Cm((size_t)n * n, zc(0, 0));
+  for (int i = 0; i < n; ++i)
+    for (int k = 0; k < n; ++k) {
+      const zc a = A[(size_t)i * n + k];
+      if (a == zc(0, 0)) continue;
+      for (int j = 0; j < n; ++j) Cm[(size_t)i * n + j] += a * B[(size_t)k * n + j];
+    }
+  return Cm;
+}
+std::vector<zc> mat_dag(const std::vector<zc>& A, int n) {
+  std::vector<zc> D((size_t)n * n);
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < n; ++j) D[(size_t)j * n + i] = std::conj(A[(size_t)i * n + j]);
+  return D;
+}
+std::vector<zc> mat_add(const std::vector<zc>& A, const std::vector<zc>& B) {
+  std::vector<zc> Cm(A.size());
+  for (size_t i = 0; i < A.size(); ++i) Cm[i] = A[i] + B[i];
+  return Cm;
+}
+
+template <typename T>
+cudaError_t upload_vec(T** dst, const void* src, size_t count) {
+  *dst = nullptr;
+  cudaError_t e = cudaMalloc((void**)dst, sizeof(T) * std::max<size_t>(count, 1));
+  if (e != cudaSuccess) return e;
+  if (count == 0) return cudaSuccess;
+  return cudaMemcpy(*dst, src, sizeof(T) * count, cudaMemcpyHostToDevice);
+}
+
+}  // namespace
+
+void block_path_destroy(BlockPath* bp) {
+  if (!bp) return;
+  cudaFree(bp->csr_rowptr); cudaFree(bp->csr_col); cudaFree(bp->csr_val);
+  cudaFree(bp->lead_mats); cudaFree(bp->table); cudaFree(bp->hist);
+  cudaFree(bp->partial); cudaFree(bp->scratch); cudaFree(bp->flags);
+  delete bp;
+}
+
+negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, const double2* w_eq_dev,
+                              const double2* z_neq_dev, const double* w_neq_dev, BlockPath** out) {
+  *out = nullptr;
+  const int n = cfg->block;
+  if (!blk::block_size_supported(n)) {
+    set_error("negf_create: block size %d is not instantiated in this build of libnegf_b200 "
+              "(see NEGF_BLOCK_SIZES in csrc/block_path.h)", n);
+    return NEGF_EINVAL;
+  }
+  BlockPath* bp = new (std::nothrow) BlockPath();
+  if (!bp) { set_error("negf_create: out of host memory"); return NEGF_ENOMEM; }
+  std::memset(bp, 0, sizeof(*bp));
+  bp->C = cfg->n_channels; bp->N = cfg->n_rings; bp->n = n;
+  bp->K_eq = cfg->n_eq; bp->K_neq = cfg->n_neq;
+  bp->mu_s = cfg->mu_s; bp->mu_d = cfg->mu_d; bp->kT = cfg->kT; bp->deg = cfg->deg;
+  bp->sr_tol = cfg->sr_tol; bp->sr_maxit = cfg->sr_maxit;
+  bp->z_eq = z_eq_dev; bp->w_eq = w_eq_dev; bp->z_neq = z_neq_dev; bp->w_neq = w_neq_dev;
+  auto fail = [&](negf_status st) { block_path_destroy(bp); return st; };
+
+  // ---- coupling blocks: dense copies, the four CSR matrices, the lead's constant products
+  const size_t nn = (size_t)n * n;
+  std::vector<zc> E(nn), O(nn);
+  for (size_t i = 0; i < nn; ++i) {
+    E[i] = zc(cfg->coup_even[i].re, cfg->coup_even[i].im);
+    O[i] = zc(cfg->coup_odd[i].re, cfg->coup_odd[i].im);
+  }
+  const std::vector<zc> Ed = mat_dag(E, n), Od = mat_dag(O, n);
+  const std::vector<zc>* four[4] = {&E, &Ed, &O, &Od};     // CSR_E, CSR_EDAG, CSR_O, CSR_ODAG
+  int nnz_cap = 1;
+  for (int m = 0; m < 4; ++m) {
+    int c = 0;
+    for (size_t i = 0; i < nn; ++i) c += ((*four[m])[i] != zc(0, 0));
+    nnz_cap = std::max(nnz_cap, c);
+  }
+  bp->nnz_cap = nnz_cap;
+  std::vector<int> rowptr(4 * (n + 1), 0), col((size_t)4 * nnz_cap, 0);
+  std::vector<double2> val((size_t)4 * nnz_cap, make_double2(0.0, 0.0));
+  for (int m = 0; m < 4; ++m) {
+    int e = 0;
+    for (int r = 0; r < n; ++r) {
+      rowptr[m * (n + 1) + r] = e;
+      for (int c = 0; c < n; ++c) {
+        const zc v = (*four[m])[(size_t)r * n + c];
+        if (v != zc(0, 0)) {
+          col[(size_t)m * nnz_cap + e] = c;
+          val[(size_t)m * nnz_cap + e] = make_double2(v.real(), v.imag());
+          ++e;
+        }
+      }
+    }
+    rowptr[m * (n + 1) + n] = e;
+  }
+  // lead 0 (left, rings -1, -2, ...): V0 = H_{-1,-2} = E^dagger, V1 = H_{-2,-3} = O^dagger,
+  //   Sigma_L = tau^dagger g tau with tau = H_{-1,0} = O          -> (L, R) = (O^dagger, O)
+  // lead 1 (right, rings N, N+1, ...): V0 = H_{N,N+1}, V1 = H_{N+1,N+2},
+  //   Sigma_R = H_{N-1,N} g H_{N-1,N}^dagger                     -> (L, R) = (bond(N-1), bond(N-1)^dagger)
+  auto bond = [&](int j) -> const std::vector<zc>& { return (j % 2 == 0) ? E : O; };
+  auto bond_dag = [&](int j) -> const std::vector<zc>& { return (j % 2 == 0) ? Ed : Od; };
+  std::vector<double2> lead((size_t)2 * 6 * nn);
+  for (int l = 0; l < 2; ++l) {
+    const std::vector<zc>& V0 = l == 0 ? Ed : bond(bp->N);
+    const std::vector<zc>& V1 = l == 0 ? Od : bond(bp->N + 1);
+    const std::vector<zc> V0d = mat_dag(V0, n), V1d = mat_dag(V1, n);
+    const std::vector<zc> P00 = mat_mul(V0, V0d, n);
+    const std::vector<zc> PE = mat_add(mat_mul(V1d, V1, n), P00);
+    const std::vector<zc> PA = mat_mul(V0, V1, n);
+    const std::vector<zc> PB = mat_mul(V1d, V0d, n);
+    const std::vector<zc>& Lm = l == 0 ? Od : bond(bp->N - 1);
+    const std::vector<zc>& Rm = l == 0 ? O : bond_dag(bp->N - 1);
+    const std::vector<zc>* six[6] = {&P00, &PE, &PA, &PB, &Lm, &Rm};
+    for (int m = 0; m < 6; ++m)
+      for (size_t i = 0; i < nn; ++i)
+        lead[((size_t)l * 6 + m) * nn + i] = make_double2((*six[m])[i].real(), (*six[m])[i].imag());
+  }
+  cudaError_t e = cudaSuccess;
+  auto chk = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+  chk(upload_vec(&bp->csr_rowptr, rowptr.data(), rowptr.size()));
+  chk(upload_vec(&bp->csr_col, col.data(), col.size()));
+  chk(upload_vec(&bp->csr_val, val.data(), val.size()));
+  chk(upload_vec(&bp->lead_mats, lead.data(), lead.size()));
+
+  // ---- geometry and workspace plan
+  bp->tpc = blk::block_tasks_per_cta(n);
+  bp->threads = blk::block_threads(n);
+  bp->geq = (bp->K_eq + bp->tpc - 1) / bp->tpc;
+  bp->gneq = (bp->K_neq + bp->tpc - 1) / bp->tpc;
+  bp->n_eq_cta = (long long)bp->C * bp->geq * 2;
+  bp->total_cta = (long long)bp->C * 2 * (bp->geq + bp->gneq);
+  const size_t K_all = (size_t)bp->K_eq + bp->K_neq;
+  bp->table_bytes = (int64_t)(sizeof(double2) * (size_t)bp->C * K_all * 2 * 2 * nn);
+  const int R = bp->geq + 2 * bp->gneq;
+  bp->partial_bytes = (int64_t)(sizeof(double) * (size_t)bp->C * R * bp->N);
+  const int nslice = (R + 63) / 64;
+  chk(cudaMalloc((void**)&bp->table, (size_t)bp->table_bytes));
+  chk(cudaMalloc((void**)&bp->partial, (size_t)bp->partial_bytes));
+  chk(cudaMalloc((void**)&bp->scratch, sizeof(double) * (size_t)bp->C * nslice * bp->N));
+  chk(cudaMalloc((void**)&bp->flags, 2 * sizeof(int)));
+  if (e == cudaSuccess) chk(cudaMemset(bp->flags, 0, 2 * sizeof(int)));
+  if (e != cudaSuccess) {
+    set_error("negf_create (block path): device allocation failed: %s", cudaGetErrorString(e));
+    return fail(e == cudaErrorMemoryAllocation ? NEGF_ENOMEM : NEGF_ECUDA);
+  }
+  int dev = 0, sms = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  bp->ctas_per_sm = blk::block_sweep_ctas_per_sm(n, nnz_cap);
+  if (bp->ctas_per_sm < 1) {
+    cudaGetLastError();
+    set_error("negf_create: the block sweep kernel does not fit on this device (n = %d, nnz = %d)", n, nnz_cap);
+    return fail(NEGF_ECUDA);
+  }
+  bp->wave = std::max(2, bp->ctas_per_sm * sms);
+  bp->slot_bytes = (int64_t)sizeof(double2) * bp->N * n * bp->threads;
+  size_t free_b = 0, total_b = 0;
+  cudaMemGetInfo(&free_b, &total_b);
+  int64_t budget = cfg->workspace_bytes > 0 ? cfg->workspace_bytes : (int64_t)((double)free_b * 0.85);
+  budget = std::min<int64_t>(budget, (int64_t)((double)free_b * 0.95));
+  long long slots = std::min<long long>(bp->total_cta, budget / bp->slot_bytes);
+  slots = std::min<long long>(slots, 2LL * bp->wave);
+  if (slots > bp->wave) slots = slots / bp->wave * bp->wave;
+  slots &= ~1LL;
+  if (slots < 2) {
+    set_error("negf_create: recursion-history workspace too small (need >= %lld bytes for two CTAs)",
+              (long long)(2 * bp->slot_bytes));
+    return fail(NEGF_ENOMEM);
+  }
+  bp->slots = (int)slots;
+  bp->hist_bytes = bp->slot_bytes * slots;
+  bp->n_launches = (int)((bp->total_cta + slots - 1) / slots);
+  e = cudaMalloc((void**)&bp->hist, (size_t)bp->hist_bytes);
+  if (e != cudaSuccess) {
+    set_error("negf_create: cannot allocate %lld bytes of recursion history: %s", (long long)bp->hist_bytes,
+              cudaGetErrorString(e));
+    return fail(NEGF_ENOMEM);
+  }
+  *out = bp;
+  return NEGF_OK;
+}
+
+negf_status block_path_self_energy(BlockPath* bp, const double* U_dev, cudaStream_t s, ProfHook hook) {
+  blk::SrLaunch p;
+  p.C = bp->C; p.N = bp->N; p.K_eq = bp->K_eq; p.K_neq = bp->K_neq;
+  p.U = U_dev; p.z_eq = bp->z_eq; p.z_neq = bp->z_neq;
+  p.lead_mats = bp->lead_mats; p.table = bp->table;
+  p.tol = bp->sr_tol; p.maxit = bp->sr_maxit; p.theta2 = g_theta2;
+  p.max_iters = bp->flags; p.noconv_flag = bp->flags + 1;
+  NEGF_CUDA_TRY(cudaMemsetAsync(bp->flags, 0, 2 * sizeof(int), s));
+  hook.begin(hook.ctx, 0);
+  cudaError_t e = blk::launch_sancho_rubio(bp->n, p, s);
+  hook.end(hook.ctx);
+  NEGF_CUDA_TRY(e);
+  return NEGF_OK;
+}
+
+negf_status block_path_run(BlockPath* bp, const double* U_dev, double* n_res, double* T_res,
+                           cudaStream_t s, ProfHook hook) {
+  blk::SweepLaunch p;
+  p.C = bp->C; p.N = bp->N; p.K_eq = bp->K_eq; p.K_neq = bp->K_neq;
+  p.geq = bp->geq; p.gneq = bp->gneq;
+  p.U = U_dev; p.z_eq = bp->z_eq; p.w_eq = bp->w_eq; p.z_neq = bp->z_neq; p.w_neq = bp->w_neq;
+  p.table = bp->table;
+  p.mu_s = bp->mu_s; p.mu_d = bp->mu_d; p.kT = bp->kT; p.deg = bp->deg; p.theta2 = g_theta2;
+  p.hist = bp->hist; p.partial = bp->partial; p.T = T_res;
+  p.csr.rowptr = bp->csr_rowptr; p.csr.col = bp->csr_col; p.csr.val = bp->csr_val;
+  p.csr.nnz_cap = bp->nnz_cap;
+  for (long long begin = 0; begin < bp->total_cta; begin += bp->slots) {
+    p.cta_begin = begin;
+    p.n_cta = (int)std::min<long long>(bp->slots, bp->total_cta - begin);
+    hook.begin(hook.ctx, 1);
+    cudaError_t e = blk::launch_block_sweep(bp->n, p, s);
+    hook.end(hook.ctx);
+    NEGF_CUDA_TRY(e);
+    const long long eq_end = std::min<long long>(begin + p.n_cta, bp->n_eq_cta);
+    if (eq_end > begin) {
+      hook.begin(hook.ctx, 3);
+      e = blk::launch_block_combine(bp->n, p, begin, (int)((eq_end - begin) / 2), s);
+      hook.end(hook.ctx);
+      NEGF_CUDA_TRY(e);
+    }
+  }
+  hook.begin(hook.ctx, 2);
+  cudaError_t e = launch_reduce_rows(bp->partial, n_res, bp->C, bp->geq + 2 * bp->gneq, bp->N, 1.0,
+                                     bp->scratch, s);
+  hook.end(hook.ctx);
+  NEGF_CUDA_TRY(e);
+  return NEGF_OK;
+}
+
+negf_status block_path_check(BlockPath* bp) {
+  int host[2] = {0, 0};
+  NEGF_CUDA_TRY(cudaMemcpy(host, bp->flags, sizeof(host), cudaMemcpyDeviceToHost));
+  bp->last_max_iters = host[0];
+  if (host[1]) {
+    set_error("Sancho-Rubio decimation did not reach sr_tol within sr_maxit = %d iterations for at least "
+              "one (channel, energy, lead)", bp->sr_maxit);
+    return NEGF_ENOCONV;
+  }
+  return NEGF_OK;
+}
+
+void block_path_plan(BlockPath* bp, negf_plan_info* out) {
+  out->history_bytes = bp->hist_bytes;
+  out->partial_bytes = bp->partial_bytes;
+  out->n_batches = bp->n_launches;
+  out->max_sr_iterations = bp->last_max_iters;
+}
+
 }  // namespace negf

@@ -1,14 +1,20 @@
 // Block (real-space, n x n) path: Sancho-Rubio self-energies + block RGF sweeps (configs[2..4]).
+// Host-side interface used by negf_api.cu, and the launch descriptors shared by the kernels'
+// translation units (sancho_rubio.cu, block_sweep.cu, block_path.cu).
 #pragma once
 #include <cuda_runtime.h>
 
 #include "negf.h"
 
+// Block sizes the kernels are instantiated for (registers hold one matrix row per thread, so the
+// size is a compile-time constant).  17 = (17,0) tube; the small ones serve the brute-force tests.
+#define NEGF_BLOCK_SIZES(X) X(2) X(3) X(4) X(5) X(8) X(17)
+
 namespace negf {
 
 struct BlockPath;
 
-struct ProfHook {                 // optional per-kernel timing callbacks (kinds: 0 SR, 1 sweep, 2 reduce)
+struct ProfHook {                 // optional per-kernel timing callbacks (kinds: 0 SR, 1 sweep, 2 reduce, 3 combine)
   void* ctx;
   void (*begin)(void* ctx, int kind);
   void (*end)(void* ctx);
@@ -22,5 +28,65 @@ negf_status block_path_run(BlockPath* bp, const double* U_dev, double* n_res, do
 negf_status block_path_check(BlockPath* bp);
 void block_path_plan(BlockPath* bp, negf_plan_info* out);
 void block_path_destroy(BlockPath* bp);
+void block_path_set_pivot_threshold(double theta);   // process-wide; <= 0 restores the default
 
+namespace blk {
+
+// Sparse coupling matrices on the device: four CSR matrices E, E^dagger, O, O^dagger
+// (E = coup_even = H_{i,i+1} for even i, O = coup_odd), concatenated.
+struct CsrSet {
+  const int* rowptr;     // [4][nb + 1], each starting at 0
+  const int* col;        // [4][nnz_cap]
+  const double2* val;    // [4][nnz_cap]
+  int nnz_cap;           // max nnz over the four
+};
+enum { CSR_E = 0, CSR_EDAG = 1, CSR_O = 2, CSR_ODAG = 3 };
+
+struct SrLaunch {
+  int C, N, K_eq, K_neq;
+  const double* U;            // [C][N]
+  const double2* z_eq;        // [K_eq]
+  const double2* z_neq;       // [K_neq]
+  const double2* lead_mats;   // [2 leads][6][nb*nb]: V0 V0^+, V1^+ V1 + V0 V0^+, V0 V1, V1^+ V0^+, L, R
+  double2* table;             // [C][K_eq + K_neq][2 leads][2: Sigma, F][nb*nb]
+  double tol;
+  double theta2;              // pivot acceptance threshold (block_ops.cuh)
+  int maxit;
+  int* max_iters;             // device scalar, atomicMax
+  int* noconv_flag;           // device scalar
+};
+cudaError_t launch_sancho_rubio(int nb, const SrLaunch& p, cudaStream_t s);
+
+// One launch of the sweep kernel covers the global CTA range [cta_begin, cta_begin + n_cta).
+// Global CTA numbering: contour CTAs first, (channel, energy group, direction) with direction
+// fastest, then real-axis CTAs in the same order.  CTA j of the launch owns history slot j.
+struct SweepLaunch {
+  int C, N, K_eq, K_neq;
+  int geq, gneq;              // energy groups per channel: ceil(K / TPC)
+  long long cta_begin;
+  int n_cta;
+  const double* U;
+  const double2 *z_eq, *w_eq, *z_neq;
+  const double* w_neq;
+  const double2* table;       // Sigma / F table of SrLaunch
+  double mu_s, mu_d, kT, deg;
+  double theta2;              // pivot acceptance threshold (block_ops.cuh)
+  double2* hist;              // [slots][N][nb][THREADS]
+  double* partial;            // [C][geq + 2 gneq][N]
+  double* T;                  // [C][K_neq]
+  CsrSet csr;
+};
+cudaError_t launch_block_sweep(int nb, const SweepLaunch& p, cudaStream_t s);
+// Contour combine over the pairs of contour CTAs [cta_begin, cta_begin + 2 n_pairs) of a finished
+// sweep launch whose first CTA was launch_cta_begin.
+cudaError_t launch_block_combine(int nb, const SweepLaunch& p, long long pair_cta_begin, int n_pairs,
+                                 cudaStream_t s);
+// Geometry queries (host).
+int block_tasks_per_cta(int nb);
+int block_threads(int nb);
+size_t block_sweep_smem(int nb, int nnz_cap);
+int block_sweep_ctas_per_sm(int nb, int nnz_cap);
+bool block_size_supported(int nb);
+
+}  // namespace blk
 }  // namespace negf

@@ -30,9 +30,9 @@ using namespace negf;
 
 namespace {
 
-enum KernelKind { K_SCALAR_SWEEP = 0, K_REDUCE, K_SANCHO, K_BLOCK_SWEEP, K_MISC, K_COUNT };
+enum KernelKind { K_SCALAR_SWEEP = 0, K_REDUCE, K_SANCHO, K_BLOCK_SWEEP, K_BLOCK_COMBINE, K_MISC, K_COUNT };
 const char* const kKernelNames[K_COUNT] = {"scalar_sweep", "reduce", "sancho_rubio", "block_sweep",
-                                           "misc"};
+                                           "block_combine", "misc"};
 
 struct ProfEntry {
   int kind;
@@ -129,12 +129,12 @@ void prof_collect(negf_handle* h) {
   h->prof_pending.clear();
 }
 
-// begin/end callbacks handed to the block path (kinds: 0 Sancho-Rubio, 1 sweep, 2 reduce)
+// begin/end callbacks handed to the block path (kinds: 0 Sancho-Rubio, 1 sweep, 2 reduce, 3 combine)
 void hook_begin(void* ctx, int kind) {
   negf_handle* h = static_cast<negf_handle*>(ctx);
   if (!h->profile) return;
   ProfEntry ent;
-  ent.kind = kind == 0 ? K_SANCHO : (kind == 1 ? K_BLOCK_SWEEP : K_REDUCE);
+  ent.kind = kind == 0 ? K_SANCHO : (kind == 1 ? K_BLOCK_SWEEP : (kind == 3 ? K_BLOCK_COMBINE : K_REDUCE));
   ent.a = prof_event(h);
   ent.b = prof_event(h);
   cudaEventRecord(ent.a, h->stream);
@@ -229,6 +229,10 @@ negf_status run_sweeps(negf_handle* h) {
 }  // namespace
 
 extern "C" const char* negf_last_error(void) { return negf::g_err; }
+extern "C" negf_status negf_set_pivot_threshold(double theta) {
+  negf::block_path_set_pivot_threshold(theta);
+  return NEGF_OK;
+}
 extern "C" const char* negf_version(void) { return "negf_b200 0.1 (sm_100a)"; }
 
 extern "C" negf_status negf_destroy(negf_handle* h) {

@@ -1,0 +1,164 @@
+"""GPU parity, block (real-space, n x n) path: shrunk and sampled versions of BASELINE.json
+configs[2..4] through the C-ABI against the CPU oracle, element by element (north_star: 1e-10
+relative).  Dense inversion (tier O1) on shrunk devices, the paper's recursion (tier O3) at full
+device length, random non-symmetric complex blocks to catch dagger / transpose / ordering mistakes,
+and the forced column-search path of the in-register Gauss-Jordan."""
+import numpy as np
+import pytest
+
+import workloads as wlmod
+from oracle import negf_dense as od
+from oracle import negf_rgf as orgf
+from tests.parity import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+
+def _gpu_run(wl, want_plan=False, **kw):
+    import torch
+    from paper_2407_14633_b200 import Negf
+    h = Negf.from_workload(wl, **kw)
+    phi = torch.tensor(wl.phi, dtype=torch.float64, device="cuda")
+    n = torch.empty((wl.C, wl.N), dtype=torch.float64, device="cuda")
+    T = torch.empty((wl.C, max(wl.K_neq, 1)), dtype=torch.float64, device="cuda")
+    h.negf_set_potential(phi)
+    h.negf_charge(n)
+    h.negf_transmission(T)
+    h.negf_sync()
+    out = n.cpu().numpy(), T.cpu().numpy()[:, :wl.K_neq]
+    plan = h.negf_get_plan()
+    h.negf_destroy()
+    return out + (plan,) if want_plan else out
+
+
+def _random_block_workload(n, N, K_neq, K_eq, seed, C=1, sparse=False):
+    """Device with random complex non-Hermitian coupling blocks (not a CNT): every dagger,
+    transpose and left/right ordering in the recursion matters."""
+    rng = np.random.default_rng(seed)
+    base = wlmod.make_config(3, N=N, K_neq=max(K_neq, 1), K_eq=K_eq)
+    if K_neq == 0:
+        base = base.subset(neq_idx=[])
+
+    def blockmat():
+        m = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+        if sparse:
+            m = m * (rng.uniform(size=(n, n)) < 0.4)
+            m[0, n - 1] = 1.0 + 0.5j            # keep it connected
+        return (0.9 * m).astype(np.complex128)
+
+    phi = 0.3 * rng.normal(size=(C, N))
+    return wlmod.Workload(
+        name=f"random_n{n}", kind="block", C=C, N=N, n=n, n_modes=1,
+        coup_even=blockmat(), coup_odd=blockmat(), mode_weight=np.ones(1), phi=phi,
+        z_eq=base.z_eq, w_eq=base.w_eq, z_neq=base.z_neq, w_neq=base.w_neq, lead_kind=1, seed=seed)
+
+
+@pytest.mark.parametrize("N,K_neq,K_eq", [(12, 8, 4), (33, 37, 17), (2, 5, 3), (7, 16, 0), (9, 0, 6)])
+def test_config3_shrunk_vs_dense_definition(N, K_neq, K_eq):
+    """17 x 17 blocks; several CTAs per direction (K > 15) with ragged tails, even and odd N (both
+    parities of the right lead), the degenerate N = 2, contour-only and real-axis-only handles."""
+    wl = wlmod.make_config(3, N=N, K_neq=max(K_neq, 1), K_eq=K_eq)
+    if K_neq == 0:
+        wl = wl.subset(neq_idx=[])
+    n_ref, T_ref = od.charge_and_transmission(wl)
+    n, T = _gpu_run(wl)
+    assert_parity(n, n_ref, "config3-shrunk charge")
+    if K_neq:
+        assert_parity(T, T_ref, "config3-shrunk T(E)")
+
+
+@pytest.mark.parametrize("n,sparse", [(2, False), (3, False), (4, True), (5, False), (8, True)])
+def test_random_complex_blocks_vs_dense_definition(n, sparse):
+    wl = _random_block_workload(n, N=9 + n, K_neq=40, K_eq=11, seed=100 + n, C=2, sparse=sparse)
+    n_ref, T_ref = od.charge_and_transmission(wl)
+    n_gpu, T_gpu = _gpu_run(wl)
+    assert_parity(n_gpu, n_ref, f"random n={n} charge")
+    assert_parity(T_gpu, T_ref, f"random n={n} T(E)")
+
+
+def test_forced_column_search_matches():
+    """theta = 1e150 rejects every diagonal candidate, so every elimination step takes the
+    partial-pivoting search path; the results must still match the dense definition."""
+    from paper_2407_14633_b200 import negf_set_pivot_threshold
+    wl3 = wlmod.make_config(3, N=10, K_neq=20, K_eq=5)
+    wlr = _random_block_workload(5, N=11, K_neq=17, K_eq=4, seed=77)
+    refs = [od.charge_and_transmission(w) for w in (wl3, wlr)]
+    try:
+        negf_set_pivot_threshold(1e150)
+        for w, (n_ref, T_ref) in zip((wl3, wlr), refs):
+            n, T = _gpu_run(w)
+            assert_parity(n, n_ref, f"{w.name} forced-search charge")
+            assert_parity(T, T_ref, f"{w.name} forced-search T(E)")
+    finally:
+        negf_set_pivot_threshold(0.0)
+
+
+def test_config4_shrunk_multi_channel():
+    wl = wlmod.make_config(4, C=3, N=14, K_neq=19, K_eq=5)
+    n_ref, T_ref = od.charge_and_transmission(wl)
+    n, T = _gpu_run(wl)
+    assert_parity(n, n_ref, "config4-shrunk charge")
+    assert_parity(T, T_ref, "config4-shrunk T(E)")
+
+
+def test_real_space_equals_sum_of_modes_on_gpu():
+    """Pin P7 on the GPU: the block path on the (17,0) real-space tube reproduces the scalar path
+    on its 17 mode chains (ring-uniform potential => block-circulant tube)."""
+    wl = wlmod.make_config(3, N=40, K_neq=48, K_eq=8)
+    twin = wlmod.scalar_twin(wl)
+    n_b, T_b = _gpu_run(wl)
+    n_s, T_s = _gpu_run(twin)
+    assert_parity(n_b, n_s, "block vs modes charge")
+    assert_parity(T_b, T_s, "block vs modes T(E)", rtol=2e-10)   # both sides SR/closed-form limited
+
+
+def test_workspace_tiling_gives_identical_results():
+    """A small workspace cap forces several sweep launches (contour pairs and real-axis CTAs in
+    different launches); results must be bit-identical."""
+    wl = wlmod.make_config(3, N=16, K_neq=50, K_eq=20)
+    n1, T1, plan1 = _gpu_run(wl, want_plan=True)
+    slot = 16 * 17 * 256 * 16
+    n2, T2, plan2 = _gpu_run(wl, want_plan=True, workspace_bytes=4 * slot)
+    assert plan2["n_batches"] > plan1["n_batches"] >= 1
+    assert np.array_equal(n1, n2) and np.array_equal(T1, T2)
+
+
+def test_config3_full_length_sampled_vs_paper_recursion():
+    """Full device length (N = 1000, the bench launch geometry: 256-thread CTAs, 15 tasks each) on a
+    sample of configs[2]'s energies against tier O3."""
+    wl = wlmod.config3()
+    rng = np.random.default_rng(11)
+    sub = wl.subset(neq_idx=np.sort(rng.choice(wl.K_neq, 20, replace=False)),
+                    eq_idx=np.sort(rng.choice(wl.K_eq, 4, replace=False)))
+    n_ref, T_ref = orgf.charge_and_transmission(sub, chunk=24)
+    n, T = _gpu_run(sub)
+    assert_parity(n, n_ref, "config3 sampled charge")
+    assert_parity(T, T_ref, "config3 sampled T(E)")
+
+
+def test_sancho_rubio_iterations_and_nonconvergence():
+    import torch
+    from paper_2407_14633_b200 import Negf, NegfError
+    wl = wlmod.make_config(3, N=8, K_neq=8, K_eq=2)
+    h = Negf.from_workload(wl)
+    phi = torch.tensor(wl.phi, dtype=torch.float64, device="cuda")
+    h.negf_set_potential(phi)
+    h.negf_sync()
+    its = h.negf_get_plan()["max_sr_iterations"]
+    assert 5 <= its <= 60          # eta = 1e-6: ~20 doublings, + 2 extra passes
+    h.negf_destroy()
+    wl.sr_maxit = 3
+    h = Negf.from_workload(wl)
+    h.negf_set_potential(phi)
+    with pytest.raises(NegfError) as ei:
+        h.negf_sync()
+    assert ei.value.status == 4    # NEGF_ENOCONV
+    h.negf_destroy()
+
+
+def test_unsupported_block_size_fails_loudly():
+    from paper_2407_14633_b200 import NegfError
+    wl = _random_block_workload(7, N=6, K_neq=4, K_eq=2, seed=5)
+    with pytest.raises(NegfError) as ei:
+        _gpu_run(wl)
+    assert ei.value.status == 1    # NEGF_EINVAL, no silent fallback
