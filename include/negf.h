@@ -108,6 +108,12 @@ NEGF_API negf_status negf_charge(negf_handle* h, double* n_dev);
  * cached by negf_charge, or runs the sweep itself if the potential changed since. */
 NEGF_API negf_status negf_transmission(negf_handle* h, double* T_dev);
 
+/* Lead self-energies of the current potential (step a1b; eq.(2)): copies
+ * Sigma[C][K_eq + K_neq][2 leads: 0 = source/left, 1 = drain/right][n*n row-major] (contour energies
+ * first) to sigma_dev.  Block handles (lead_kind 1) only: scalar handles evaluate the closed form
+ * inside the sweep kernel and return NEGF_EINVAL here.  NEGF_ESTATE before negf_set_potential. */
+NEGF_API negf_status negf_self_energy(negf_handle* h, negf_c64* sigma_dev);
+
 /* Landauer reductions of T(E) (eq.(5)-(6)), per channel:
  *   current[c]     = sum_k w_k T_c(E_k) (f_S(E_k) - f_D(E_k))      in eV, multiply by g_s e/h
  *   conductance[c] = sum_k w_k T_c(E_k) (-df/dE)(E_k; mu_s, kT)    in units of G_0 = g_s e^2/h

@@ -25,7 +25,7 @@ STATUS_NAMES = {0: "NEGF_OK", 1: "NEGF_EINVAL", 2: "NEGF_ENOMEM", 3: "NEGF_ECUDA
 # every symbol include/negf.h declares (tests check the library exports all of them)
 EXPORTED_SYMBOLS = [
     "negf_create", "negf_destroy", "negf_set_potential", "negf_charge", "negf_transmission",
-    "negf_current", "negf_solve_host", "negf_sync", "negf_kernel_stats", "negf_get_plan",
+    "negf_self_energy", "negf_current", "negf_solve_host", "negf_sync", "negf_kernel_stats", "negf_get_plan",
     "broyden_create", "broyden_step", "broyden_reset", "broyden_destroy",
     "negf_fp64_peak", "negf_set_pivot_threshold", "negf_last_error", "negf_version",
 ]
@@ -85,6 +85,7 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
         "negf_set_potential": (C.c_int, [vp, vp]),
         "negf_charge": (C.c_int, [vp, vp]),
         "negf_transmission": (C.c_int, [vp, vp]),
+        "negf_self_energy": (C.c_int, [vp, vp]),
         "negf_current": (C.c_int, [vp, vp, vp]),
         "negf_solve_host": (C.c_int, [vp, vp, vp, vp]),
         "negf_sync": (C.c_int, [vp]),
@@ -203,6 +204,14 @@ class Negf:
     def negf_transmission(self, T_dev):
         _check(self._lib.negf_transmission(self._h, _dev_ptr(T_dev, self.C * self.K_neq, "T_dev")),
                "negf_transmission")
+
+    def negf_self_energy(self, sigma_dev):
+        """sigma_dev: complex128 CUDA tensor [C][K_eq + K_neq][2][n*n]."""
+        import torch
+        if (not isinstance(sigma_dev, torch.Tensor) or not sigma_dev.is_cuda
+                or sigma_dev.dtype != torch.complex128 or not sigma_dev.is_contiguous()):
+            raise ValueError("sigma_dev: need a contiguous complex128 CUDA tensor")
+        _check(self._lib.negf_self_energy(self._h, C.c_void_p(sigma_dev.data_ptr())), "negf_self_energy")
 
     def negf_current(self, current_dev=None, conductance_dev=None):
         a = _dev_ptr(current_dev, self.C, "current_dev") if current_dev is not None else None

@@ -148,7 +148,7 @@ negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, c
   //   Sigma_R = H_{N-1,N} g H_{N-1,N}^dagger                     -> (L, R) = (bond(N-1), bond(N-1)^dagger)
   auto bond = [&](int j) -> const std::vector<zc>& { return (j % 2 == 0) ? E : O; };
   auto bond_dag = [&](int j) -> const std::vector<zc>& { return (j % 2 == 0) ? Ed : Od; };
-  std::vector<double2> lead((size_t)2 * 6 * nn);
+  std::vector<double2> lead((size_t)2 * blk::kLeadMats * nn);
   for (int l = 0; l < 2; ++l) {
     const std::vector<zc>& V0 = l == 0 ? Ed : bond(bp->N);
     const std::vector<zc>& V1 = l == 0 ? Od : bond(bp->N + 1);
@@ -159,10 +159,10 @@ negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, c
     const std::vector<zc> PB = mat_mul(V1d, V0d, n);
     const std::vector<zc>& Lm = l == 0 ? Od : bond(bp->N - 1);
     const std::vector<zc>& Rm = l == 0 ? O : bond_dag(bp->N - 1);
-    const std::vector<zc>* six[6] = {&P00, &PE, &PA, &PB, &Lm, &Rm};
-    for (int m = 0; m < 6; ++m)
+    const std::vector<zc>* all[blk::kLeadMats] = {&P00, &PE, &PA, &PB, &Lm, &Rm, &V0, &V1, &V0d, &V1d};
+    for (int m = 0; m < blk::kLeadMats; ++m)
       for (size_t i = 0; i < nn; ++i)
-        lead[((size_t)l * 6 + m) * nn + i] = make_double2((*six[m])[i].real(), (*six[m])[i].imag());
+        lead[((size_t)l * blk::kLeadMats + m) * nn + i] = make_double2((*all[m])[i].real(), (*all[m])[i].imag());
   }
   cudaError_t e = cudaSuccess;
   auto chk = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
@@ -275,6 +275,15 @@ negf_status block_path_run(BlockPath* bp, const double* U_dev, double* n_res, do
                                      bp->scratch, s);
   hook.end(hook.ctx);
   NEGF_CUDA_TRY(e);
+  return NEGF_OK;
+}
+
+negf_status block_path_copy_sigma(BlockPath* bp, double2* sigma_dev, cudaStream_t s) {
+  // table entry = [Sigma | F], n*n each: strided copy of the Sigma halves
+  const size_t nn = (size_t)bp->n * bp->n;
+  const size_t entries = (size_t)bp->C * ((size_t)bp->K_eq + bp->K_neq) * 2;
+  NEGF_CUDA_TRY(cudaMemcpy2DAsync(sigma_dev, nn * sizeof(double2), bp->table, 2 * nn * sizeof(double2),
+                                  nn * sizeof(double2), entries, cudaMemcpyDeviceToDevice, s));
   return NEGF_OK;
 }
 

@@ -26,6 +26,7 @@ negf_status block_path_self_energy(BlockPath* bp, const double* U_dev, cudaStrea
 negf_status block_path_run(BlockPath* bp, const double* U_dev, double* n_res, double* T_res,
                            cudaStream_t s, ProfHook hook);
 negf_status block_path_check(BlockPath* bp);
+negf_status block_path_copy_sigma(BlockPath* bp, double2* sigma_dev, cudaStream_t s);
 void block_path_plan(BlockPath* bp, negf_plan_info* out);
 void block_path_destroy(BlockPath* bp);
 void block_path_set_pivot_threshold(double theta);   // process-wide; <= 0 restores the default
@@ -42,12 +43,14 @@ struct CsrSet {
 };
 enum { CSR_E = 0, CSR_EDAG = 1, CSR_O = 2, CSR_ODAG = 3 };
 
+constexpr int kLeadMats = 10;
 struct SrLaunch {
   int C, N, K_eq, K_neq;
   const double* U;            // [C][N]
   const double2* z_eq;        // [K_eq]
   const double2* z_neq;       // [K_neq]
-  const double2* lead_mats;   // [2 leads][6][nb*nb]: V0 V0^+, V1^+ V1 + V0 V0^+, V0 V1, V1^+ V0^+, L, R
+  const double2* lead_mats;   // [2 leads][kLeadMats][nb*nb]: V0 V0^+, V1^+ V1 + V0 V0^+, V0 V1, V1^+ V0^+,
+                              //   L, R, V0, V1, V0^+, V1^+
   double2* table;             // [C][K_eq + K_neq][2 leads][2: Sigma, F][nb*nb]
   double tol;
   double theta2;              // pivot acceptance threshold (block_ops.cuh)

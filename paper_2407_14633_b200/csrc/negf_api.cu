@@ -373,6 +373,16 @@ extern "C" negf_status negf_transmission(negf_handle* h, double* T_dev) {
   return NEGF_OK;
 }
 
+extern "C" negf_status negf_self_energy(negf_handle* h, negf_c64* sigma_dev) {
+  if (!h || !sigma_dev) { set_error("negf_self_energy: null argument"); return NEGF_EINVAL; }
+  if (h->scalar) {
+    set_error("negf_self_energy: scalar handles evaluate the closed form inside the sweep kernel");
+    return NEGF_EINVAL;
+  }
+  if (!h->have_potential) { set_error("no potential set: call negf_set_potential first"); return NEGF_ESTATE; }
+  return block_path_copy_sigma(h->block, reinterpret_cast<double2*>(sigma_dev), h->stream);
+}
+
 extern "C" negf_status negf_current(negf_handle* h, double* current_dev, double* conductance_dev) {
   if (!h) { set_error("negf_current: null handle"); return NEGF_EINVAL; }
   negf_status st = run_sweeps(h);

@@ -3,15 +3,29 @@
 // Gamma = i (Sigma - Sigma^dagger) = F F^dagger that the sweep kernel propagates.
 //
 // The lead is a semi-infinite stack of rings r0 (surface), r1, r2, ... with uniform on-site energy
-// U and alternating hoppings V0 = H_{r0,r1}, V1 = H_{r1,r2}, V0, ...  Because every on-site block is
-// U I, the odd rings are eliminated in closed form first (w = 1/(z - U)):
-//     eps_s = U + w V0 V0^dagger,   eps = U + w (V1^dagger V1 + V0 V0^dagger),
-//     a = w V0 V1,                  b = w V1^dagger V0^dagger,
-// which leaves an n x n chain (not the 2n x 2n principal layer) for the decimation loop
-//     g = (z - eps)^-1;  eps_s += a g b;  eps += a g b + b g a;  a <- a g a;  b <- b g b
-// until max|a_ij|, |b_ij| < sr_tol, plus two more passes (quadratic convergence: the fixed point is
-// then exact to rounding, so the result does not depend on the route taken to it).
-// g_surf = (z - eps_s)^-1,  Sigma = L g_surf R  with (L, R) = (tau^dagger, tau).
+// U and alternating hoppings V0 = H_{r0,r1}, V1 = H_{r1,r2}, V0, ...  Its principal layer is the
+// two-ring cell (r0, r1):  H00 = [[U, V0], [V0^+, U]],  H01 = [[0, 0], [V1, 0]].  Cells must hold an
+// even number of rings: segments with an odd number of rings of a bipartite chain carry zero modes
+// at z = U, so any decimation that isolates them (e.g. eliminating every other ring first) is
+// singular in the middle of the energy window.
+//
+// Because H01 has a single non-zero n x n block, the decimation matrices keep that shape for ever,
+//     a = |1> X <0|,  b = |0> Y <1|,   X = V1, Y = V1^+ initially,
+// and with g = (z - eps)^-1 (2n x 2n, four n x n blocks g00 g01 g10 g11) one pass is
+//     eps_11 += X g00 Y;  eps_s,11 += X g00 Y;  eps_00 += Y g11 X;  X <- X g01 X;  Y <- Y g10 Y,
+// the off-diagonal blocks of eps staying V0, V0^+.  So the only 2n x 2n operation is the inversion;
+// the eight products are n x n.  Loop until max|X_ij|, |Y_ij| < sr_tol, plus two more passes.
+//
+// Thread geometry: 2n threads per task, thread (h, a) owns row h n + a of the 2n x 2n matrix during
+// the inversion (block_ops.cuh gj_invert<2n>) and row a of the n x n blocks of half h otherwise.
+//
+// The raw decimation is conditioning-limited (it inverts isolated 2^k-cell segments whose poles lie
+// on the real axis, eta away from z): 1e-13 typical, 1e-8 next to such a pole.  It is therefore
+// polished with Newton steps on the surface block X = g_surf,00, the only part the next cell sees:
+//     G(X) = [z - H00 - |1> V1 X V1^+ <1|]^-1,   F(X) = G00 - X = 0,
+//     dG00 = P dX Q,  P = G01 V1,  Q = V1^+ G10,   D - P D Q = G00 - X  summed by doubling
+//     (D += P D Q;  P <- P^2;  Q <- Q^2),
+// until the fixed-point residual is at rounding level (at most kNewtonMax passes).
 #include "block_ops.cuh"
 #include "block_path.h"
 #include "negf_internal.h"
@@ -19,23 +33,63 @@
 namespace negf {
 namespace blk {
 
+constexpr int kNewtonMax = 4;
+
+// c[b] = sum_k arow[k] * X[k * LD + b]
+template <int NB, int LD>
+__device__ __forceinline__ void gemm_row_ld(c64 (&c)[NB], const c64 (&arow)[NB], const c64* X) {
+#pragma unroll
+  for (int b = 0; b < NB; ++b) c[b] = make_double2(0.0, 0.0);
+#pragma unroll
+  for (int k = 0; k < NB; ++k) {
+    const c64 av = arow[k];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) cfma(c[b], av, X[k * LD + b]);
+  }
+}
 template <int NB>
-__global__ void __launch_bounds__(Geo<NB>::THREADS, 1) sancho_rubio_kernel(const SrLaunch p) {
-  using G = Geo<NB>;
+__device__ __forceinline__ void row_from(c64 (&r)[NB], const c64* src) {
+#pragma unroll
+  for (int b = 0; b < NB; ++b) r[b] = src[b];
+}
+template <int NB>
+__device__ __forceinline__ void row_to(c64* dst, const c64 (&r)[NB], bool pred) {
+  if (!pred) return;
+#pragma unroll
+  for (int b = 0; b < NB; ++b) dst[b] = r[b];
+}
+template <int NB>
+__device__ __forceinline__ double row_absmax(const c64 (&r)[NB]) {
+  double m = 0.0;
+#pragma unroll
+  for (int b = 0; b < NB; ++b) m = fmax(m, fmax(fabs(r[b].x), fabs(r[b].y)));
+  return m;
+}
+
+template <int NB>
+__global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(const SrLaunch p) {
+  constexpr int N2 = 2 * NB;
+  using G2 = Geo<N2>;
+  constexpr int MATN = NB * NB;
   extern __shared__ __align__(16) char smem_raw[];
-  Smem<NB> sm;
-  sm.carve(smem_raw, 3);
+  Smem<N2> sm;
+  char* nxt = sm.carve(smem_raw, 1);
   const int tid = threadIdx.x;
-  const bool live = tid < G::LIVE;
-  const int t = live ? tid / NB : 0;
-  const int a = tid % NB;
-  c64* bufG = sm.mat + (size_t)t * G::MAT;
-  c64* bufA = sm.mat + ((size_t)G::TPC + t) * G::MAT;
-  c64* bufB = sm.mat + ((size_t)2 * G::TPC + t) * G::MAT;
+  const bool live = tid < G2::LIVE;
+  const int t = live ? tid / N2 : 0;
+  const int r = tid % N2;
+  const int h = r / NB;            // 0: rows of ring r0, 1: rows of ring r1
+  const int a = r - h * NB;
+  const bool live0 = live && h == 0;
+  c64* Gt = sm.mat + (size_t)t * G2::MAT;                          // 2n x 2n, leading dimension N2
+  c64* Xb = reinterpret_cast<c64*>(nxt) + (size_t)t * 2 * MATN;    // n x n
+  c64* Yb = Xb + MATN;                                             // n x n
+  c64* mine = h == 0 ? Yb : Xb;    // half 0 carries Y (-> eps_00, new Y), half 1 carries X
+  c64* other = h == 0 ? Xb : Yb;
 
   const int K_all = p.K_eq + p.K_neq;
   const long long n_task = (long long)p.C * K_all * 2;
-  long long task = (long long)blockIdx.x * G::TPC + t;
+  long long task = (long long)blockIdx.x * G2::TPC + t;
   const bool active = live && task < n_task;
   if (task >= n_task) task = n_task - 1;
   const int lead = (int)(task & 1);
@@ -44,86 +98,74 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 1) sancho_rubio_kernel(const
   const int kk = (int)(ck - (long long)c * K_all);
   const c64 z = kk < p.K_eq ? p.z_eq[kk] : p.z_neq[kk - p.K_eq];
   const double U = p.U[(size_t)c * p.N + (lead ? p.N - 1 : 0)];
-  const c64 w = crcp(make_double2(z.x - U, z.y));
-  const c64* lm = p.lead_mats + (size_t)lead * 6 * G::MAT;   // P00, PE, PA, PB, L, R (row-major)
+  const c64* lm = p.lead_mats + (size_t)lead * kLeadMats * MATN;   // see block_path.h
+  const c64* gL = lm + 4 * MATN;
+  const c64* gR = lm + 5 * MATN;
+  const c64* gV0 = lm + 6 * MATN;
+  const c64* gV1 = lm + 7 * MATN;
+  const c64* gV0d = lm + 8 * MATN;
+  const c64* gV1d = lm + 9 * MATN;
+  // this thread's row of the constant off-diagonal block of z - eps: -V0 (half 0) / -V0^+ (half 1)
+  const c64* offrow = (h == 0 ? gV0 : gV0d) + a * NB;
+  const c64* my_init = (h == 0 ? gV1d : gV1) + a * NB;
 
-  c64 eps_s[NB], eps[NB];
+  // row r of z - eps:  half 0: [z - eps_00 | -V0],  half 1: [-V0^+ | z - eps_11]
+  auto build_row = [&](c64 (&m)[N2], const c64 (&ediag)[NB]) {
+#pragma unroll
+    for (int j = 0; j < NB; ++j) {
+      const c64 dg = make_double2((j == a ? z.x : 0.0) - ediag[j].x, (j == a ? z.y : 0.0) - ediag[j].y);
+      const c64 of = offrow[j];
+      const c64 no = make_double2(-of.x, -of.y);
+      m[j] = h == 0 ? dg : no;
+      m[NB + j] = h == 0 ? no : dg;
+    }
+  };
+
+  c64 eh[NB];          // row a of eps_hh
+  c64 es[NB];          // row a of eps_s,11 (half 1; half 0 keeps eps_s,00 = U I)
 #pragma unroll
   for (int b = 0; b < NB; ++b) {
-    eps_s[b] = cmul(w, lm[0 * G::MAT + a * NB + b]);
-    eps[b] = cmul(w, lm[1 * G::MAT + a * NB + b]);
-    if (b == a) { eps_s[b].x += U; eps[b].x += U; }
-    if (live) {
-      bufA[a * NB + b] = cmul(w, lm[2 * G::MAT + a * NB + b]);
-      bufB[a * NB + b] = cmul(w, lm[3 * G::MAT + a * NB + b]);
-    }
+    eh[b] = make_double2(b == a ? U : 0.0, 0.0);
+    es[b] = eh[b];
+    if (live) mine[a * NB + b] = my_init[b];
   }
-  int remaining = -1;       // -1: criterion not met yet; >= 0: passes still to do after it was met
+  int remaining = -1;  // -1: criterion not met yet; >= 0: passes still to do after it was met
   int iters = 0;
   bool frozen = false;
   __syncthreads();
 
   for (int it = 0; it < p.maxit + 2; ++it) {
-    c64 d[NB];
-#pragma unroll
-    for (int b = 0; b < NB; ++b) d[b] = make_double2((b == a ? z.x : 0.0) - eps[b].x, (b == a ? z.y : 0.0) - eps[b].y);
-    const bool permuted = gj_invert<NB>(d, sm, t, a, live, p.theta2);
-    store_inverse<NB>(d, bufG, sm, t, a, live, permuted);
+    {
+      c64 m[N2];
+      build_row(m, eh);
+      const bool permuted = gj_invert<N2>(m, sm, t, r, live, p.theta2);
+      store_inverse<N2>(m, Gt, sm, t, r, live, permuted);
+    }
     __syncthreads();
-    c64 ag[NB], bg[NB];
-    {
-      c64 row[NB];
-#pragma unroll
-      for (int k = 0; k < NB; ++k) row[k] = bufA[a * NB + k];
-      gemm_row<NB>(ag, row, bufG);
-#pragma unroll
-      for (int k = 0; k < NB; ++k) row[k] = bufB[a * NB + k];
-      gemm_row<NB>(bg, row, bufG);
-    }
-    __syncthreads();                       // bufG is free from here on
-    double rowmax = 0.0;
-    c64 nb_[NB];
-    {
-      c64 tmp[NB];
-      gemm_row<NB>(tmp, ag, bufB);         // a g b
-      if (!frozen) {
-#pragma unroll
-        for (int b = 0; b < NB; ++b) {
-          eps_s[b].x += tmp[b].x; eps_s[b].y += tmp[b].y;
-          eps[b].x += tmp[b].x;   eps[b].y += tmp[b].y;
-        }
-      }
-      gemm_row<NB>(tmp, bg, bufA);         // b g a
-      if (!frozen) {
-#pragma unroll
-        for (int b = 0; b < NB; ++b) { eps[b].x += tmp[b].x; eps[b].y += tmp[b].y; }
-      }
-      gemm_row<NB>(tmp, ag, bufA);         // a g a -> new a, parked in bufG
+    const int rb = (1 - h) * NB;   // half 0 works on g11 / g10, half 1 on g00 / g01
+    c64 ar[NB], pq[NB], res[NB];
+    row_from<NB>(ar, mine + a * NB);
+    gemm_row_ld<NB, N2>(pq, ar, Gt + rb * N2 + rb);          // Y g11   | X g00
+    gemm_row<NB>(res, pq, other);                            // Y g11 X | X g00 Y
+    if (!frozen) {
 #pragma unroll
       for (int b = 0; b < NB; ++b) {
-        if (frozen) tmp[b] = make_double2(0.0, 0.0);
-        rowmax = fmax(rowmax, fmax(fabs(tmp[b].x), fabs(tmp[b].y)));
-        if (live) bufG[a * NB + b] = tmp[b];
-      }
-      gemm_row<NB>(nb_, bg, bufB);         // b g b -> new b
-#pragma unroll
-      for (int b = 0; b < NB; ++b) {
-        if (frozen) nb_[b] = make_double2(0.0, 0.0);
-        rowmax = fmax(rowmax, fmax(fabs(nb_[b].x), fabs(nb_[b].y)));
+        eh[b].x += res[b].x; eh[b].y += res[b].y;
+        es[b].x += res[b].x; es[b].y += res[b].y;            // only meaningful for half 1
       }
     }
-    if (live) sm.mag[t * NB + a] = rowmax;
-    __syncthreads();                       // everyone is done reading bufA / bufB
+    gemm_row_ld<NB, N2>(pq, ar, Gt + rb * N2 + (NB - rb));   // Y g10   | X g01
+    gemm_row<NB>(res, pq, mine);                             // Y g10 Y | X g01 X
+    if (frozen) {
 #pragma unroll
-    for (int b = 0; b < NB; ++b) {
-      if (live) {
-        bufB[a * NB + b] = nb_[b];
-        bufA[a * NB + b] = bufG[a * NB + b];   // own row only
-      }
+      for (int b = 0; b < NB; ++b) res[b] = make_double2(0.0, 0.0);
     }
+    if (live) sm.mag[t * N2 + r] = row_absmax<NB>(res);
+    __syncthreads();                                         // all reads of Gt, Xb, Yb done
+    row_to<NB>(mine + a * NB, res, live);
     double tmax = 0.0;
 #pragma unroll
-    for (int i = 0; i < NB; ++i) tmax = fmax(tmax, sm.mag[t * NB + i]);
+    for (int i = 0; i < N2; ++i) tmax = fmax(tmax, sm.mag[t * N2 + i]);
     if (!frozen) {
       ++iters;
       if (remaining < 0) {
@@ -135,41 +177,164 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 1) sancho_rubio_kernel(const
     }
     if (__syncthreads_and(frozen || !live)) break;
   }
-  if (active && a == 0) {
+  if (active && r == 0) {
     atomicMax(p.max_iters, iters);
     if (!frozen) atomicExch(p.noconv_flag, 1);
   }
 
-  // ---- surface Green's function and Sigma = L g R
+  // ---- surface Green's function of the layer: (z - eps_s)^-1, eps_s,00 = U I
+  {
+    c64 m[N2], ed[NB];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) ed[b] = h == 0 ? make_double2(b == a ? U : 0.0, 0.0) : es[b];
+    build_row(m, ed);
+    const bool permuted = gj_invert<N2>(m, sm, t, r, live, p.theta2);
+    store_inverse<N2>(m, Gt, sm, t, r, live, permuted);
+#pragma unroll
+    for (int b = 0; b < NB; ++b)
+      if (live) mine[a * NB + b] = my_init[b];               // Xb = V1, Yb = V1^+ again
+  }
+  __syncthreads();
+
+  // ---- Newton polish of X = g_surf,00 (header).  Gt holds a full inverse whose 00 block is X.
+  c64* Pb = Gt;                    // staging inside Gt once the inverse has been consumed
+  c64* Qb = Gt + MATN;
+  c64* Tb = Gt + 2 * MATN;
+  double final_res = 0.0, final_scale = 1.0;
+  for (int pass = 0; pass < kNewtonMax; ++pass) {
+    c64 gold[NB];                  // row a of X (half 0)
+    {
+      c64 m[N2], ed[NB];
+      if (h == 0) {
+        row_from<NB>(gold, Gt + a * N2);
+#pragma unroll
+        for (int b = 0; b < NB; ++b) ed[b] = make_double2(b == a ? U : 0.0, 0.0);
+      } else {
+        c64 ar[NB], w1[NB];
+        row_from<NB>(ar, Xb + a * NB);                       // V1 row a
+        gemm_row_ld<NB, N2>(w1, ar, Gt);                     // V1 X
+        gemm_row<NB>(ed, w1, Yb);                            // V1 X V1^+
+#pragma unroll
+        for (int b = 0; b < NB; ++b)
+          if (b == a) ed[b].x += U;
+      }
+      build_row(m, ed);
+      const bool permuted = gj_invert<N2>(m, sm, t, r, live, p.theta2);
+      store_inverse<N2>(m, Gt, sm, t, r, live, permuted);    // Gt = G(X)
+    }
+    __syncthreads();
+    c64 dlt[NB];                   // half 0: residual row, then the Newton correction
+    c64 pqrow[NB];                 // half 0: row a of P;  half 1: row a of Q
+    if (h == 0) {
+      c64 ar[NB];
+#pragma unroll
+      for (int b = 0; b < NB; ++b) {
+        const c64 gn = Gt[a * N2 + b];
+        dlt[b] = make_double2(gn.x - gold[b].x, gn.y - gold[b].y);
+        ar[b] = Gt[a * N2 + NB + b];                         // G01 row a
+      }
+      gemm_row<NB>(pqrow, ar, Xb);                           // P = G01 V1
+      if (live) {
+        sm.mag[t * N2 + a] = row_absmax<NB>(dlt);
+        sm.mag[t * N2 + NB + a] = row_absmax<NB>(gold);
+      }
+    } else {
+      c64 ar[NB];
+      row_from<NB>(ar, Yb + a * NB);                         // V1^+ row a
+      gemm_row_ld<NB, N2>(pqrow, ar, Gt + NB * N2);          // Q = V1^+ G10
+#pragma unroll
+      for (int b = 0; b < NB; ++b) dlt[b] = make_double2(0.0, 0.0);
+    }
+    __syncthreads();                                         // reads of Gt done; mag visible
+    double tres = 0.0, tg = 0.0;
+#pragma unroll
+    for (int i = 0; i < NB; ++i) {
+      tres = fmax(tres, sm.mag[t * N2 + i]);
+      tg = fmax(tg, sm.mag[t * N2 + NB + i]);
+    }
+    final_res = tres;
+    final_scale = tg;
+    const bool good = tres <= 2e-14 * tg;
+    if (__syncthreads_and(good || !live)) break;            // Gt still holds G(X): X = its 00 block
+    // stage P and Q inside Gt (the inverse is dead from here)
+    row_to<NB>((h == 0 ? Pb : Qb) + a * NB, pqrow, live);
+    __syncthreads();
+    bool pdone = false;
+    for (int it = 0; it < p.maxit + 2; ++it) {
+      c64 w[NB];
+      if (h == 0) {
+        gemm_row<NB>(w, dlt, Qb);                            // D Q
+        row_to<NB>(Tb + a * NB, w, live);
+      } else {
+        gemm_row<NB>(w, pqrow, Qb);                          // Q^2
+#pragma unroll
+        for (int b = 0; b < NB; ++b) pqrow[b] = pdone ? make_double2(0.0, 0.0) : w[b];
+      }
+      __syncthreads();
+      double rowmax = 0.0;
+      c64 p2[NB];
+      if (h == 0) {
+        gemm_row<NB>(w, pqrow, Tb);                          // P D Q
+        if (!pdone) {
+#pragma unroll
+          for (int b = 0; b < NB; ++b) { dlt[b].x += w[b].x; dlt[b].y += w[b].y; }
+        }
+      } else {
+        c64 ar[NB];
+        row_from<NB>(ar, Pb + a * NB);
+        gemm_row<NB>(p2, ar, Pb);                            // P^2 (computed by half 1 to balance the work)
+        if (pdone) {
+#pragma unroll
+          for (int b = 0; b < NB; ++b) p2[b] = make_double2(0.0, 0.0);
+        }
+        rowmax = fmax(row_absmax<NB>(p2), row_absmax<NB>(pqrow));
+      }
+      if (live) sm.mag[t * N2 + r] = rowmax;
+      __syncthreads();                                       // reads of Pb, Qb, Tb done
+      if (h == 1) {
+        row_to<NB>(Pb + a * NB, p2, live);
+        row_to<NB>(Qb + a * NB, pqrow, live);
+      }
+      double tmax = 0.0;
+#pragma unroll
+      for (int i = 0; i < N2; ++i) tmax = fmax(tmax, sm.mag[t * N2 + i]);
+      if (tmax < 1e-4) pdone = true;                         // |P_j| |Q_j| < 1e-8: series summed
+      const bool all_done = __syncthreads_and(pdone || !live);
+      if (h == 0) row_from<NB>(pqrow, Pb + a * NB);
+      if (all_done) break;
+    }
+    // X <- X + D, written where the next pass (or the code below) expects the 00 block
+    __syncthreads();
+    if (live0) {
+#pragma unroll
+      for (int b = 0; b < NB; ++b) Gt[a * N2 + b] = make_double2(gold[b].x + dlt[b].x, gold[b].y + dlt[b].y);
+    }
+    __syncthreads();
+  }
+  if (active && r == 0 && !(final_res <= 1e-9 * final_scale)) atomicExch(p.noconv_flag, 1);
+
+  // ---- Sigma = L g00 R  (rows owned by half 0)
   c64 srow[NB];
   {
-    c64 d[NB];
-#pragma unroll
-    for (int b = 0; b < NB; ++b)
-      d[b] = make_double2((b == a ? z.x : 0.0) - eps_s[b].x, (b == a ? z.y : 0.0) - eps_s[b].y);
-    const bool permuted = gj_invert<NB>(d, sm, t, a, live, p.theta2);
-    store_inverse<NB>(d, bufG, sm, t, a, live, permuted);
-#pragma unroll
-    for (int b = 0; b < NB; ++b)
-      if (live) bufA[a * NB + b] = lm[5 * G::MAT + a * NB + b];     // R
-    __syncthreads();
     c64 grow[NB], t1[NB];
+    row_from<NB>(grow, Gt + a * N2);
+    __syncthreads();                                         // everyone has its row of g00
+    if (live0) {
 #pragma unroll
-    for (int k = 0; k < NB; ++k) grow[k] = bufG[a * NB + k];
-    gemm_row<NB>(t1, grow, bufA);                                    // g R
-#pragma unroll
-    for (int b = 0; b < NB; ++b)
-      if (live) bufB[a * NB + b] = t1[b];
+      for (int b = 0; b < NB; ++b) Yb[a * NB + b] = gR[a * NB + b];
+    }
     __syncthreads();
-#pragma unroll
-    for (int k = 0; k < NB; ++k) grow[k] = lm[4 * G::MAT + a * NB + k];   // L row
-    gemm_row<NB>(srow, grow, bufB);                                  // L g R
+    gemm_row<NB>(t1, grow, Yb);                              // g00 R
+    row_to<NB>(Xb + a * NB, t1, live0);
+    __syncthreads();
+    row_from<NB>(grow, gL + a * NB);
+    gemm_row<NB>(srow, grow, Xb);                            // L g00 R
   }
-  c64* out = p.table + (size_t)task * 2 * G::MAT;
+  c64* out = p.table + (size_t)task * 2 * MATN;
 #pragma unroll
   for (int b = 0; b < NB; ++b) {
-    if (active) out[a * NB + b] = srow[b];
-    if (live) bufG[a * NB + b] = srow[b];
+    if (active && h == 0) out[a * NB + b] = srow[b];
+    if (live0) Yb[a * NB + b] = srow[b];
   }
   __syncthreads();
 
@@ -177,7 +342,7 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 1) sancho_rubio_kernel(const
   c64 S[NB], F[NB];
 #pragma unroll
   for (int b = 0; b < NB; ++b) {
-    const c64 sba = bufG[b * NB + a];
+    const c64 sba = Yb[b * NB + a];
     S[b] = make_double2(-(srow[b].y + sba.y), srow[b].x - sba.x);
     F[b] = make_double2(0.0, 0.0);
   }
@@ -188,17 +353,17 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 1) sancho_rubio_kernel(const
 #pragma unroll
     for (int b = 0; b < NB; ++b)
       if (b == a) diag = S[b].x;
-    if (live) sm.mag[t * NB + a] = usedc ? -1.0 : diag;
+    if (live0) sm.mag[t * N2 + a] = usedc ? -1.0 : diag;
     __syncthreads();
     int piv = 0;
-    double dmax = sm.mag[t * NB];
+    double dmax = sm.mag[t * N2];
 #pragma unroll
     for (int i = 1; i < NB; ++i) {
-      const double v = sm.mag[t * NB + i];
+      const double v = sm.mag[t * N2 + i];
       if (v > dmax) { dmax = v; piv = i; }
     }
-    c64* prow = sm.prow + ((size_t)(j & 1) * G::TPC + t) * NB;
-    if (a == piv && live) {
+    c64* prow = sm.prow + ((size_t)(j & 1) * G2::TPC + t) * N2;
+    if (a == piv && live0) {
 #pragma unroll
       for (int b = 0; b < NB; ++b) prow[b] = S[b];
     }
@@ -223,23 +388,24 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 1) sancho_rubio_kernel(const
   }
 #pragma unroll
   for (int b = 0; b < NB; ++b)
-    if (active) out[G::MAT + a * NB + b] = F[b];
+    if (active && h == 0) out[MATN + a * NB + b] = F[b];
+}
+
+template <int NB>
+static size_t sr_smem_t() {
+  return Smem<2 * NB>::bytes(1) + sizeof(c64) * (size_t)Geo<2 * NB>::TPC * 2 * NB * NB + 32;
 }
 
 template <int NB>
 static cudaError_t launch_sr_t(const SrLaunch& p, cudaStream_t s) {
-  using G = Geo<NB>;
-  const size_t smem = Smem<NB>::bytes(3);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(sancho_rubio_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)smem);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  using G2 = Geo<2 * NB>;
+  const size_t smem = sr_smem_t<NB>();
+  cudaError_t e = cudaFuncSetAttribute(sancho_rubio_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)smem);
+  if (e != cudaSuccess) return e;
   const long long n_task = (long long)p.C * (p.K_eq + p.K_neq) * 2;
-  const int blocks = (int)((n_task + G::TPC - 1) / G::TPC);
-  sancho_rubio_kernel<NB><<<blocks, G::THREADS, smem, s>>>(p);
+  const int blocks = (int)((n_task + G2::TPC - 1) / G2::TPC);
+  sancho_rubio_kernel<NB><<<blocks, G2::THREADS, smem, s>>>(p);
   return cudaGetLastError();
 }
 
