@@ -63,6 +63,8 @@ struct negf_handle {
   char* hist;
   int64_t hist_bytes, partial_bytes;
   double *partial, *scratch, *T_part;
+  cudaStream_t side;        // contour tasks run beside the real-axis tasks (fork / join by events)
+  cudaEvent_t ev_fork, ev_join;
   // results
   double *n_res, *T_res;
   // host staging for negf_solve_host
@@ -150,7 +152,7 @@ ProfHook prof_hook(negf_handle* h) { return ProfHook{h, hook_begin, hook_end}; }
 negf_status plan_scalar(negf_handle* h) {
   const int64_t N = h->N;
   h->rwarps_per_channel = (h->n_modes * h->K_neq + 31) / 32;
-  h->cwarps_per_channel = (h->n_modes * h->K_eq + 31) / 32;
+  h->cwarps_per_channel = 2 * ((h->n_modes * h->K_eq + 31) / 32);   // (group, direction) pairs
   const int wpc = h->cwarps_per_channel + 2 * h->rwarps_per_channel;
   const int64_t total = (int64_t)h->C * wpc;
   if (total <= 0 || total > (int64_t)1 << 30) {
@@ -166,7 +168,8 @@ negf_status plan_scalar(negf_handle* h) {
   int begin = 0;
   for (int w = 0; w < h->total_warps; ++w) {
     const int64_t b = (w % wpc) < h->cwarps_per_channel ? cbytes : rbytes;
-    if (acc + b > budget) {
+    const bool second_of_pair = (w % wpc) < h->cwarps_per_channel && ((w % wpc) & 1);
+    if (acc + b > budget && !second_of_pair) {
       h->batches.push_back({begin, w});
       maxacc = std::max(maxacc, acc);
       begin = w;
@@ -180,6 +183,9 @@ negf_status plan_scalar(negf_handle* h) {
   h->partial_bytes = (int64_t)h->total_warps * N * 8;
   NEGF_CUDA_TRY(cudaMalloc((void**)&h->hist, (size_t)h->hist_bytes));
   NEGF_CUDA_TRY(cudaMalloc((void**)&h->partial, (size_t)h->partial_bytes));
+  NEGF_CUDA_TRY(cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking));
+  NEGF_CUDA_TRY(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+  NEGF_CUDA_TRY(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
   const int nslice = (wpc + 63) / 64;
   NEGF_CUDA_TRY(cudaMalloc((void**)&h->scratch, sizeof(double) * (size_t)h->C * nslice * N));
   NEGF_CUDA_TRY(cudaMalloc((void**)&h->T_part,
@@ -205,6 +211,7 @@ negf_status run_sweeps(negf_handle* h) {
     p.hist_r = reinterpret_cast<double*>(h->hist);
     p.hist_c = reinterpret_cast<double2*>(h->hist);
     p.partial = h->partial; p.T_part = h->T_part;
+    p.side = h->side; p.ev_fork = h->ev_fork; p.ev_join = h->ev_join;
     for (const Batch& b : h->batches) {
       p.warp_begin = b.warp_begin;
       p.warp_end = b.warp_end;
@@ -245,6 +252,9 @@ extern "C" negf_status negf_destroy(negf_handle* h) {
   cudaFree(h->U); cudaFree(h->hist); cudaFree(h->partial); cudaFree(h->scratch);
   cudaFree(h->T_part); cudaFree(h->n_res); cudaFree(h->T_res); cudaFree(h->phi_stage);
   if (h->block) block_path_destroy(h->block);
+  if (h->side) cudaStreamDestroy(h->side);
+  if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+  if (h->ev_join) cudaEventDestroy(h->ev_join);
   delete h;
   return NEGF_OK;
 }

@@ -22,12 +22,12 @@ void set_error(const char* fmt, ...);
 // ---------------------------------------------------------------- scalar (mode-space) path
 // One half-sweep task = (channel, mode, energy, direction); a warp holds 32 tasks of the same
 // channel and direction.  Warp numbering inside a launch:
-//   [0, n_cwarps)                      contour tasks (one thread does both passes)
+//   [0, n_cwarps)                      contour tasks, even = left-to-right, odd = right-to-left
 //   [n_cwarps, n_cwarps + 2*n_rwarps)  real-axis tasks, even = left-to-right, odd = right-to-left
 struct ScalarLaunch {
   int C, N, n_modes, K_eq, K_neq;
   int rwarps_per_channel;   // ceil(n_modes*K_neq/32)
-  int cwarps_per_channel;   // ceil(n_modes*K_eq/32)
+  int cwarps_per_channel;   // 2 * ceil(n_modes*K_eq/32)
   const double* U;          // [C][N] on-site energy = -phi
   const double* bsq_even;   // [n_modes] |H_{i,i+1}|^2, i even
   const double* bsq_odd;    // [n_modes]
@@ -43,6 +43,8 @@ struct ScalarLaunch {
   double* partial;          // [total warps][N] per-warp partial charge
   double* T_part;           // [C][n_modes][K_neq]
   int warp_begin, warp_end; // global warp range of this launch
+  cudaStream_t side;        // host only: stream of the contour kernel (forked from / joined to s)
+  cudaEvent_t ev_fork, ev_join;
 };
 cudaError_t launch_scalar_sweep(const ScalarLaunch& p, cudaStream_t s);
 

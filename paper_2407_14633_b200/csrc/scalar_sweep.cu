@@ -5,9 +5,11 @@
 // independent half-sweep tasks, one per direction.  A task runs the connected-Green's-function
 // recursion of Algorithm 2 away from its first lead,
 //     g_s = 1 / (z - U_i - |beta|^2 g_{s-1}),            (ytilde / xtilde of Alg.2 for scalars)
-// stores only r_s = |g_s|^2 (8 B) per ring, then walks back with the column recursion of Algorithm 1
-// steps 2-3, which for scalars needs only moduli:
-//     |G_(i,k)|^2 = r_i |beta|^2 |G_(i+-1,k)|^2,         k = index of the task's last lead,
+// in homogeneous coordinates g_s = P_s / P_{s+1} (a three-term recurrence, no division on the
+// dependent chain), stores only h_s = |P_s|^2 (8 B) per ring, then walks
+// back with the column recursion of Algorithm 1 steps 2-3, which for scalars
+// needs only moduli and telescopes:
+//     |G_(i,k)|^2 = |g_i|^2 |beta|^2 |G_(i+-1,k)|^2 = h_i (prod |beta|^2) / |D|^2,   k = last lead,
 // giving Tr A_l,(i,i) = Gamma_l |G_(i,k)|^2 and, at the far end, T(E) (eq.(5)).
 // Contour points need the complex diagonal G_(i,i) = [alpha_i - x_i - y_i]^-1 (Alg.1 step 1) and run
 // as single tasks (right-connected pass stored as complex, left-connected pass on the fly).
@@ -19,7 +21,7 @@ namespace negf {
 namespace {
 
 constexpr int kTile = 16;           // ring steps per transposed warp reduction
-constexpr int kWarpsPerBlock = 4;
+constexpr int kWarpsPerBlock = 2;
 constexpr double kPi = 3.14159265358979323846;
 
 struct cplx {
@@ -88,31 +90,31 @@ __device__ __forceinline__ void flush_tile(double (*tile)[33], int lane, int cnt
   __syncwarp();
 }
 
-__global__ void __launch_bounds__(kWarpsPerBlock * 32, 8)
-scalar_sweep_kernel(const ScalarLaunch p) {
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 16)
+scalar_real_kernel(const ScalarLaunch p, const int n_warps) {
   __shared__ double tiles[kWarpsPerBlock][kTile][33];
   const int lane = threadIdx.x & 31;
   const int wib = threadIdx.x >> 5;
-  const int w = p.warp_begin + blockIdx.x * kWarpsPerBlock + wib;   // global warp index
-  if (w >= p.warp_end) return;
+  const int ord = blockIdx.x * kWarpsPerBlock + wib;      // ordinal among this launch's real-axis warps
+  if (ord >= n_warps) return;
   double(*tile)[33] = tiles[wib];
 
   const int N = p.N;
   const int wpc = p.cwarps_per_channel + 2 * p.rwarps_per_channel;
-  const int c = w / wpc;
-  const int local = w - c * wpc;
+  auto cw_before = [&](int ww) { return (ww / wpc) * p.cwarps_per_channel + min(ww % wpc, p.cwarps_per_channel); };
+  const int cw0 = cw_before(p.warp_begin);
+  const int g = (p.warp_begin - cw0) + ord;               // global real-axis warp ordinal
+  const int c = g / (2 * p.rwarps_per_channel);
+  const int local = p.cwarps_per_channel + (g - c * 2 * p.rwarps_per_channel);
+  const int w = c * wpc + local;                          // global warp index
   const double* __restrict__ U = p.U + (size_t)c * N;
   double* __restrict__ prow = p.partial + (size_t)w * N;
-
   // history offset of this warp inside the launch's workspace
-  auto cw_before = [&](int ww) { return (ww / wpc) * p.cwarps_per_channel + min(ww % wpc, p.cwarps_per_channel); };
-  const long long cwb = cw_before(w) - cw_before(p.warp_begin);
+  const long long cwb = cw_before(w) - cw0;
   const long long rwb = (long long)(w - p.warp_begin) - cwb;
   char* hbase = reinterpret_cast<char*>(p.hist_r) + (cwb * 16 + rwb * 8) * (long long)N * 32;
-
   const double U0 = __ldg(U), UN = __ldg(U + N - 1);
-
-  if (local >= p.cwarps_per_channel) {
+  {
     // ------------------------------------------------------------------ real-axis half-sweep task
     const int rl = local - p.cwarps_per_channel;
     const int dir = rl & 1;                 // 0: left -> right (last lead = drain), 1: right -> left
@@ -143,127 +145,247 @@ scalar_sweep_kernel(const ScalarLaunch p) {
                                  : 0.0;
 
     double* __restrict__ hist = reinterpret_cast<double*>(hbase) + lane;
-    // bond type (0 even, 1 odd) joining phase-1 steps s-1 and s:
+    // Bond type (0 even, 1 odd) joining steps s-1 and s of this direction:
     //   dir 0: bond (i-1, i), i = s      -> parity of s-1
     //   dir 1: bond (i, i+1), i = N-1-s  -> parity of N-1-s
-    const int par0 = dir ? ((N - 1) & 1) : 1;    // bond type at s = 0 (unused), flips every step
-    // ---- phase 1: connected Green's function away from the first lead (Alg.2)
-    double gre, gim, r;
-    {
-      const int i0 = dir ? N - 1 : 0;
-      double dre = z.re - __ldg(U + i0) - sig_first.re;
-      double dim = z.im - sig_first.im;
-      r = 1.0 / (dre * dre + dim * dim);
-      gre = dre * r;
-      gim = -dim * r;
-      hist[0] = r;
-    }
+    // i.e. type(s) = par0 ^ (s & 1) with par0 the (virtual) type at s = 0.
+    const int par0 = dir ? ((N - 1) & 1) : 1;
+    const double b2_odd_s = par0 ? be : bo;      // |bond|^2 entering odd steps s
+    const double b2_even_s = par0 ? bo : be;     // |bond|^2 entering even steps s >= 2
     const int istep = dir ? -1 : 1;
-    int i = dir ? N - 2 : 1;
-    int par = par0 ^ 1;
-#pragma unroll 4
-    for (int s = 1; s < N - 1; ++s, i += istep, par ^= 1) {
-      const double b2 = par ? bo : be;
-      double dre = (z.re - __ldg(U + i)) - b2 * gre;
-      double dim = z.im - b2 * gim;
-      r = 1.0 / (dre * dre + dim * dim);
-      gre = dre * r;
-      gim = -dim * r;
-      hist[(size_t)s * 32] = r;
-    }
+    const int i0 = dir ? N - 1 : 0;
+
+    // ---- phase 1: left-connected recursion of Alg.2 in homogeneous (division-free) form.
+    // With g_s = P_s / P_{s+1} the recursion g_s = 1/(alpha_s - b2_s g_{s-1}) becomes
+    //     P_{s+1} = alpha_s P_s - b2_s P_{s-1},   P_0 = 1,  P_1 = alpha_0 - Sigma_first,
+    // and the product of |ytilde|^2 that Alg.1 steps 2-3 need telescopes:
+    //     prod_{s=i}^{N-2} b2_{s+1} |g_s|^2 = (prod b2) |P_i|^2 / |P_{N-1}|^2.
+    // Only h_s = |P_s|^2 is stored (8 B per ring).  |P| is kept in range by exact power-of-two
+    // rescaling, checked every 4 steps; a rescaled step stores -h_s as the marker the way back reads.
+    double pr = 1.0, pi_ = 0.0, qr = 0.0, qi = 0.0;       // P_s, P_{s-1}
+    hist[0] = 1.0;
     {
-      const double b2 = par ? bo : be;
-      double dre = (z.re - __ldg(U + i)) - b2 * gre - sig_last.re;
-      double dim = z.im - b2 * gim - sig_last.im;
-      r = 1.0 / (dre * dre + dim * dim);     // |G_(k,k)|^2 at the last lead's ring
-      hist[(size_t)(N - 1) * 32] = r;
+      const double ar = z.re - __ldg(U + i0) - sig_first.re;
+      const double ai = z.im - sig_first.im;
+      qr = pr; qi = pi_;
+      pr = ar; pi_ = ai;                                   // P_1 = alpha_0 * 1
     }
-    // ---- phase 2: column recursion back towards the first lead (Alg.1 steps 2-3, moduli only)
-    // step q handles phase-1 step s = N-1-q; |G_(i,k)|^2 = r_s * |bond(s, s+1)|^2 * |G_(i',k)|^2.
+    int i = i0 + istep;
+    double m = fma(pr, pr, pi_ * pi_);                     // |P_1|^2
+    int s = 1;
+    // Invariant at the top of a step: (pr,pi_) = P_s, (qr,qi) = P_{s-1}, m = |P_s|^2 (negative if
+    // P_s was just rescaled), i = ring of step s.  A step stores h_s and produces P_{s+1}.
+#define NEGF_STEP(B2)                                                      \
+    {                                                                      \
+      hist[(size_t)s * 32] = m;                                            \
+      const double ar = z.re - __ldg(U + i);                               \
+      const double nr = fma(ar, pr, fma(-z.im, pi_, -(B2) * qr));          \
+      const double ni = fma(ar, pi_, fma(z.im, pr, -(B2) * qi));           \
+      qr = pr; qi = pi_; pr = nr; pi_ = ni;                                \
+      m = fma(pr, pr, pi_ * pi_);                                          \
+      i += istep; ++s;                                                     \
+    }
+#define NEGF_RANGE()                                                       \
+    {                                                                      \
+      const unsigned ex = (unsigned)(__double2hiint(m) >> 20) - 623u;      \
+      if (ex > 800u && m > 0.0) {                                          \
+        const bool big = ex < 0x80000000u;                                 \
+        const double sc = big ? 0x1p-200 : 0x1p200;                        \
+        pr *= sc; pi_ *= sc; qr *= sc; qi *= sc;                           \
+        m = -(m * (big ? 0x1p-400 : 0x1p400));                             \
+      }                                                                    \
+    }
+    // steps s = 1 .. N-2 produce P_2 .. P_{N-1}; step s uses the bond entering step s.
+    while (s + 3 < N - 1) {                                // s is odd at the top
+      NEGF_STEP(b2_odd_s)
+      NEGF_STEP(b2_even_s)
+      NEGF_STEP(b2_odd_s)
+      NEGF_STEP(b2_even_s)
+      NEGF_RANGE()
+    }
+    while (s < N - 1) {
+      const double b2 = (s & 1) ? b2_odd_s : b2_even_s;
+      NEGF_STEP(b2)
+      NEGF_RANGE()
+    }
+#undef NEGF_STEP
+#undef NEGF_RANGE
+    // here s == N-1 (or N == 2: s == 1 == N-1): (pr,pi_) = P_{N-1}, m = +-|P_{N-1}|^2
+    hist[(size_t)(N - 1) * 32] = m;
+    double c2;
+    {
+      const double b2 = ((N - 1) & 1) ? b2_odd_s : b2_even_s;
+      const double ar = z.re - __ldg(U + i) - sig_last.re;
+      const double ai = z.im - sig_last.im;
+      // D = (alpha_{N-1} - Sigma_last) P_{N-1} - b2 P_{N-2};  G_(k,k) = P_{N-1} / D
+      const double dr = fma(ar, pr, fma(-ai, pi_, -b2 * qr));
+      const double di = fma(ar, pi_, fma(ai, pr, -b2 * qi));
+      c2 = 1.0 / fma(dr, dr, di * di);
+    }
+    // ---- phase 2: column recursion back towards the first lead (Alg.1 steps 2-3, moduli only):
+    // |G_(i,k)|^2 = F_s h_s with F_{N-1} = 1/|D|^2, F_{s-1} = F_s * b2_s (* 2^-+400 across a marker).
     const int ring0 = dir ? 0 : N - 1;
     const int sign = dir ? 1 : -1;
-    double c2 = 1.0;
-    // bond between steps s and s+1 has the type computed for step s+1: par(s+1) = par0 ^ ((s+1)&1)
     for (int q0 = 0; q0 < N; q0 += kTile) {
       const int cnt = min(kTile, N - q0);
       double h[kTile];
 #pragma unroll
       for (int t = 0; t < kTile; ++t) {
-        const int s = N - 1 - (q0 + t);
-        h[t] = (t < cnt) ? hist[(size_t)s * 32] : 0.0;
+        const int ss = N - 1 - (q0 + t);
+        h[t] = (t < cnt) ? hist[(size_t)ss * 32] : 0.0;
       }
 #pragma unroll
       for (int t = 0; t < kTile; ++t) {
-        const int q = q0 + t;
-        const int s = N - 1 - q;
-        const int pt = par0 ^ ((s + 1) & 1);
-        const double b2 = (q == 0) ? 1.0 : (pt ? bo : be);
-        c2 *= h[t] * b2;
-        tile[t][lane] = (t < cnt) ? w_last * c2 : 0.0;
-        if (t == cnt - 1 && q == N - 1 && dir == 0 && active) {
-          // G_(0,N-1): transmission (eq.(5)), a4
-          p.T_part[((size_t)c * p.n_modes + mode) * p.K_neq + k] = __ldg(p.mode_w_T + mode) * gamL * gamR * c2;
+        const int ss = N - 1 - (q0 + t);
+        const double hv = fabs(h[t]);
+        const double g2 = c2 * hv;                         // |G_(i,k)|^2
+        tile[t][lane] = (t < cnt) ? w_last * g2 : 0.0;
+        if (t < cnt) {
+          if (ss == 0 && dir == 0 && active) {
+            // G_(0,N-1): transmission (eq.(5)), a4
+            p.T_part[((size_t)c * p.n_modes + mode) * p.K_neq + k] = __ldg(p.mode_w_T + mode) * gamL * gamR * g2;
+          }
+          if (h[t] < 0.0) c2 *= (hv >= 1.0) ? 0x1p-400 : 0x1p400;
+          c2 *= (ss & 1) ? b2_odd_s : b2_even_s;           // bond entering step ss
         }
       }
       flush_tile(tile, lane, cnt, prow, ring0 + sign * q0, sign);
     }
-  } else {
-    // ------------------------------------------------------------------ contour task
+  }
+}
+
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 8)
+scalar_contour_kernel(const ScalarLaunch p, const int n_warps) {
+  __shared__ double tiles[kWarpsPerBlock][kTile][33];
+  const int lane = threadIdx.x & 31;
+  const int wib = threadIdx.x >> 5;
+  const int ord = blockIdx.x * kWarpsPerBlock + wib;      // ordinal among this launch's contour warps
+  if (ord >= n_warps) return;
+  double(*tile)[33] = tiles[wib];
+
+  const int N = p.N;
+  const int wpc = p.cwarps_per_channel + 2 * p.rwarps_per_channel;
+  auto cw_before = [&](int ww) { return (ww / wpc) * p.cwarps_per_channel + min(ww % wpc, p.cwarps_per_channel); };
+  const int cw0 = cw_before(p.warp_begin);
+  const int g = cw0 + ord;                                // global contour warp ordinal
+  const int c = g / p.cwarps_per_channel;
+  const int local = g - c * p.cwarps_per_channel;
+  const int w = c * wpc + local;                          // global warp index
+  const double* __restrict__ U = p.U + (size_t)c * N;
+  double* __restrict__ prow = p.partial + (size_t)w * N;
+  // history offset of this warp inside the launch's workspace
+  const long long cwb = cw_before(w) - cw0;
+  const long long rwb = (long long)(w - p.warp_begin) - cwb;
+  char* hbase = reinterpret_cast<char*>(p.hist_r) + (cwb * 16 + rwb * 8) * (long long)N * 32;
+  const double U0 = __ldg(U), UN = __ldg(U + N - 1);
+  {
+    // ------------------------------------------------------------------ contour half-sweep task
+    // local = 2 * group + direction.  Direction 0 stores y_i (left-connected), direction 1 stores x_i
+    // (right-connected), both indexed by ring; scalar_combine_kernel then forms G_(i,i) (Alg.1 step 1).
+    (void)tile; (void)prow;
+    const int dir = local & 1;
+    const int grp = local >> 1;
     const int ntask = p.n_modes * p.K_eq;
-    int e = local * 32 + lane;
-    const bool active = e < ntask;
-    if (!active) e = ntask - 1;
+    int e = grp * 32 + lane;
+    if (e >= ntask) e = ntask - 1;
     const int mode = e / p.K_eq;
     const int k = e - mode * p.K_eq;
     const cplx z = {p.z_eq[k].x, p.z_eq[k].y};
-    const cplx W = {p.w_eq[k].x, p.w_eq[k].y};
     const double be = __ldg(p.bsq_even + mode), bo = __ldg(p.bsq_odd + mode);
-    const double tauL2 = bo, t1L2 = be;
-    const double tauR2 = ((N - 1) & 1) ? bo : be, t1R2 = ((N - 1) & 1) ? be : bo;
-    cplx gl = surface_gf_alternating({z.re - U0, z.im}, sqrt(t1L2), sqrt(tauL2));
-    cplx gr = surface_gf_alternating({z.re - UN, z.im}, sqrt(t1R2), sqrt(tauR2));
-    const cplx sigL = {tauL2 * gl.re, tauL2 * gl.im};
-    const cplx sigR = {tauR2 * gr.re, tauR2 * gr.im};
-    const double wc = active ? -__ldg(p.mode_w + mode) / kPi : 0.0;   // deg * mode_weight * (-1/pi)
-
+    cplx sig_first;
+    if (dir == 0) {
+      const cplx gl = surface_gf_alternating({z.re - U0, z.im}, sqrt(be), sqrt(bo));
+      sig_first = {bo * gl.re, bo * gl.im};
+    } else {
+      const double tauR2 = ((N - 1) & 1) ? bo : be, t1R2 = ((N - 1) & 1) ? be : bo;
+      const cplx gr = surface_gf_alternating({z.re - UN, z.im}, sqrt(t1R2), sqrt(tauR2));
+      sig_first = {tauR2 * gr.re, tauR2 * gr.im};
+    }
     double2* __restrict__ hist = reinterpret_cast<double2*>(hbase) + lane;
-    // pass 1: x_i = |beta_i|^2 gR_{i+1} for i = N-2..0 (right-connected, Alg.2 xtilde); store x_i
-    cplx x = sigR;                                   // plays the role of x_{N-1} (lead instead of a ring)
-    for (int i = N - 1; i >= 1; --i) {
-      cplx d = {z.re - __ldg(U + i) - x.re, z.im - x.im};
-      cplx g = crcp(d);
-      const double b2 = ((i - 1) & 1) ? bo : be;     // bond (i-1, i)
-      x = {b2 * g.re, b2 * g.im};
-      hist[(size_t)(i - 1) * 32] = make_double2(x.re, x.im);
-    }
-    // pass 2: y_i on the fly (left-connected), G_ii = 1/(alpha_i - x_i - y_i)  (Alg.1 step 1)
-    cplx y = sigL;
-    for (int q0 = 0; q0 < N; q0 += kTile) {
-      const int cnt = min(kTile, N - q0);
-#pragma unroll 4
-      for (int t = 0; t < kTile; ++t) {
-        const int i = q0 + t;
-        double v = 0.0;
-        if (t < cnt) {
-          cplx xi;
-          if (i < N - 1) {
-            double2 hx = hist[(size_t)i * 32];
-            xi = {hx.x, hx.y};
-          } else {
-            xi = sigR;
-          }
-          const double u = __ldg(U + i);
-          cplx dl = {z.re - u - y.re, z.im - y.im};            // alpha_i - y_i
-          cplx G = crcp({dl.re - xi.re, dl.im - xi.im});        // G_ii
-          v = wc * (W.re * G.im + W.im * G.re);                 // -(deg/pi) Im(W G)
-          cplx gL = crcp(dl);
-          const double b2 = (i & 1) ? bo : be;                  // bond (i, i+1)
-          y = {b2 * gL.re, b2 * gL.im};
+    const int par0 = dir ? ((N - 1) & 1) : 1;       // bond type entering step s is par0 ^ (s & 1)
+    const double b2_odd_s = par0 ? be : bo;
+    const double b2_even_s = par0 ? bo : be;
+    const int istep = dir ? -1 : 1;
+    int i = dir ? N - 1 : 0;
+    // Homogeneous form of Alg.2 (see scalar_real_kernel): P_{s+1} = alpha_s P_s - b2_s P_{s-1} keeps the
+    // dependent chain free of divisions; the stored quantity y_s = b2_s g_{s-1} = b2_s P_{s-1} / P_s
+    // (x_i for direction 1) is formed off the chain and is invariant under the power-of-two rescaling.
+    hist[(size_t)i * 32] = make_double2(sig_first.re, sig_first.im);   // the lead plays ring "-1"
+    double qr = 1.0, qi = 0.0;                                          // P_0
+    double pr = z.re - __ldg(U + i) - sig_first.re, pi_ = z.im - sig_first.im;   // P_1
+    i += istep;
+    for (int s = 1; s < N; ++s, i += istep) {
+      const double b2 = (s & 1) ? b2_odd_s : b2_even_s;
+      // y_s = b2 P_{s-1} conj(P_s) / |P_s|^2
+      const double m = fma(pr, pr, pi_ * pi_);
+      const double r = b2 / m;
+      const double tr = fma(qr, pr, qi * pi_), ti = fma(qi, pr, -qr * pi_);
+      hist[(size_t)i * 32] = make_double2(tr * r, ti * r);
+      const double ar = z.re - __ldg(U + i);
+      double nr = fma(ar, pr, fma(-z.im, pi_, -b2 * qr));
+      double ni = fma(ar, pi_, fma(z.im, pr, -b2 * qi));
+      qr = pr; qi = pi_; pr = nr; pi_ = ni;
+      if ((s & 3) == 0) {
+        const unsigned ex = (unsigned)(__double2hiint(m) >> 20) - 623u;
+        if (ex > 800u && m > 0.0) {
+          const double sc = (ex < 0x80000000u) ? 0x1p-200 : 0x1p200;
+          pr *= sc; pi_ *= sc; qr *= sc; qi *= sc;
         }
-        tile[t][lane] = v;
       }
-      flush_tile(tile, lane, cnt, prow, q0, 1);
     }
+  }
+}
+
+// Contour combine: G_(i,i) = 1 / (alpha_i - x_i - y_i) (Alg.1 step 1) and the first term
+// of eq.(4): -(deg/pi) Im[W_k G_(i,i)], summed over the 32 (mode, energy) tasks of a warp pair.
+// grid = (ring chunks of 32 * kWarpsPerBlock... see launcher, pairs); one warp per (pair, 32 rings).
+__global__ void __launch_bounds__(128)
+scalar_combine_kernel(const ScalarLaunch p, const int n_pairs) {
+  __shared__ double tiles[4][32][33];
+  const int lane = threadIdx.x & 31;
+  const int wib = threadIdx.x >> 5;
+  const int pair = blockIdx.y;
+  const int N = p.N;
+  const int i0 = (blockIdx.x * 4 + wib) * 32;
+  if (i0 >= N) return;
+  const int wpc = p.cwarps_per_channel + 2 * p.rwarps_per_channel;
+  auto cw_before = [&](int ww) { return (ww / wpc) * p.cwarps_per_channel + min(ww % wpc, p.cwarps_per_channel); };
+  const int cw0 = cw_before(p.warp_begin);
+  const int g = cw0 + 2 * pair;                            // global contour warp ordinal of direction 0
+  const int c = g / p.cwarps_per_channel;
+  const int local = g - c * p.cwarps_per_channel;
+  const int w = c * wpc + local;
+  const double* __restrict__ U = p.U + (size_t)c * N;
+  const long long cwb = cw_before(w) - cw0;
+  const long long rwb = (long long)(w - p.warp_begin) - cwb;
+  const char* hbase = reinterpret_cast<const char*>(p.hist_r) + (cwb * 16 + rwb * 8) * (long long)N * 32;
+  const double2* __restrict__ hy = reinterpret_cast<const double2*>(hbase) + lane;
+  const double2* __restrict__ hx = hy + (size_t)N * 32;   // the direction-1 warp follows directly
+
+  const int ntask = p.n_modes * p.K_eq;
+  int e = (local >> 1) * 32 + lane;
+  const bool active = e < ntask;
+  if (!active) e = ntask - 1;
+  const int mode = e / p.K_eq;
+  const int k = e - mode * p.K_eq;
+  const cplx z = {p.z_eq[k].x, p.z_eq[k].y};
+  const cplx W = {p.w_eq[k].x, p.w_eq[k].y};
+  const double wc = active ? -__ldg(p.mode_w + mode) / kPi : 0.0;   // deg * mode_weight * (-1/pi)
+  double(*tile)[33] = tiles[wib];
+  const int cnt = min(32, N - i0);
+  for (int t = 0; t < cnt; ++t) {
+    const int i = i0 + t;
+    const double2 y = hy[(size_t)i * 32], x = hx[(size_t)i * 32];
+    const cplx G = crcp({z.re - __ldg(U + i) - x.x - y.x, z.im - x.y - y.y});
+    tile[t][lane] = wc * (W.re * G.im + W.im * G.re);
+  }
+  __syncwarp();
+  double acc = 0.0;
+  if (lane < cnt) {
+#pragma unroll
+    for (int j = 0; j < 32; ++j) acc += tile[lane][j];
+    p.partial[(size_t)w * N + i0 + lane] = acc;
+    p.partial[(size_t)(w + 1) * N + i0 + lane] = 0.0;      // the direction-1 warp's row carries nothing
   }
 }
 
@@ -272,9 +394,35 @@ scalar_sweep_kernel(const ScalarLaunch p) {
 cudaError_t launch_scalar_sweep(const ScalarLaunch& p, cudaStream_t s) {
   const int nwarps = p.warp_end - p.warp_begin;
   if (nwarps <= 0) return cudaSuccess;
-  const int blocks = (nwarps + kWarpsPerBlock - 1) / kWarpsPerBlock;
-  scalar_sweep_kernel<<<blocks, kWarpsPerBlock * 32, 0, s>>>(p);
-  return cudaGetLastError();
+  const int wpc = p.cwarps_per_channel + 2 * p.rwarps_per_channel;
+  auto cw_before = [&](int ww) {
+    const int r = ww % wpc;
+    return (ww / wpc) * p.cwarps_per_channel + (r < p.cwarps_per_channel ? r : p.cwarps_per_channel);
+  };
+  const int n_c = cw_before(p.warp_end) - cw_before(p.warp_begin);
+  const int n_r = nwarps - n_c;
+  // The few contour warps are latency-bound (two dependent passes over N rings); they start first on
+  // the side stream and the real-axis kernel fills the rest of the machine beside them.
+  cudaError_t e;
+  if (n_c > 0) {
+    if ((e = cudaEventRecord(p.ev_fork, s)) != cudaSuccess) return e;
+    if ((e = cudaStreamWaitEvent(p.side, p.ev_fork, 0)) != cudaSuccess) return e;
+    scalar_contour_kernel<<<(n_c + kWarpsPerBlock - 1) / kWarpsPerBlock, kWarpsPerBlock * 32, 0, p.side>>>(p, n_c);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if ((e = cudaEventRecord(p.ev_join, p.side)) != cudaSuccess) return e;
+  }
+  if (n_r > 0) {
+    scalar_real_kernel<<<(n_r + kWarpsPerBlock - 1) / kWarpsPerBlock, kWarpsPerBlock * 32, 0, s>>>(p, n_r);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  }
+  if (n_c > 0) {
+    if ((e = cudaStreamWaitEvent(s, p.ev_join, 0)) != cudaSuccess) return e;
+    if (n_c & 1) return cudaErrorInvalidValue;             // batches never split a contour pair
+    dim3 grid((p.N + 127) / 128, n_c / 2);
+    scalar_combine_kernel<<<grid, 128, 0, s>>>(p, n_c / 2);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  }
+  return cudaSuccess;
 }
 
 }  // namespace negf
