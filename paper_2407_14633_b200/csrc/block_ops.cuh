@@ -61,7 +61,7 @@ struct Csr {
 template <int NB>
 struct Smem {
   c64* mat;      // [TPC][NB*NB]   one exchange matrix per task
-  c64* prow;     // [2][TPC][NB]   published pivot rows (double buffered by elimination step)
+  c64* prow;     // [2][TPC][NB+1] published pivot rows + inverse pivot (double buffered by elimination step)
   double* mag;   // [TPC][NB]      pivot-search magnitudes / small per-task reductions
   int* pk;       // [2][TPC]       pivot row of the current elimination step
   int* perm;     // [TPC][NB]      pivot row chosen for column k
@@ -70,7 +70,7 @@ struct Smem {
 
   static constexpr size_t bytes(int nmat = 1) {
     using G = Geo<NB>;
-    return sizeof(c64) * ((size_t)nmat * G::TPC * G::MAT + 2 * G::TPC * NB) +
+    return sizeof(c64) * ((size_t)nmat * G::TPC * G::MAT + 2 * G::TPC * (NB + 1)) +
            sizeof(double) * (G::TPC * NB + 2 * G::NWARPS) + sizeof(int) * (2 * G::TPC + G::TPC * NB + G::TPC) + 64;
   }
   // returns the first byte after the carved region (16-byte aligned)
@@ -78,7 +78,7 @@ struct Smem {
     using G = Geo<NB>;
     mat = reinterpret_cast<c64*>(base);
     prow = mat + (size_t)nmat * G::TPC * G::MAT;
-    mag = reinterpret_cast<double*>(prow + 2 * G::TPC * NB);
+    mag = reinterpret_cast<double*>(prow + 2 * G::TPC * (NB + 1));
     red = mag + G::TPC * NB;
     pk = reinterpret_cast<int*>(red + 2 * G::NWARPS);
     perm = pk + 2 * G::TPC;
@@ -88,12 +88,16 @@ struct Smem {
   }
 };
 
-// Default threshold of the diagonal-candidate test in gj_invert: the candidate pivot is accepted
-// when |a_kk|^2 >= theta2 * max_j |a_kj|^2 (normalised pivot-row entries bounded by 1/theta = 1e3);
-// otherwise the task falls back to a full column search over its unused rows.
+// Default threshold of the diagonal-candidate test in gj_invert: the candidate pivot a_kk is accepted
+// when |a_kk|^2 >= theta2 * max_j |a_kj(0)|^2 (row k of the matrix as handed in); otherwise the task
+// falls back to a full column search over its unused rows (partial pivoting).
 constexpr double kTheta2Default = 1e-6;
 
 // In-place Gauss-Jordan inversion of the task's matrix, rows in registers (r = row `a`).
+// The pivot row is NOT normalised during the elimination (that would be a divergent n-element
+// scaling by one thread per step): its owner publishes the raw row with a 1 in the pivot column plus
+// the reciprocal pivot; every other row forms its multiplier f = a_ik / a_kk itself and eliminates;
+// all rows are scaled by their own reciprocal pivot once at the end.
 // Pivoting is implicit (rows never move): on return, thread i holds row q(i) of the inverse with
 // column j of its registers being inverse column perm[j], where perm[k] is the pivot row chosen for
 // column k and q = perm^-1.  Returns (CTA-uniform) whether any task left the diagonal pivot order; if
@@ -104,31 +108,30 @@ template <int NB>
 __device__ __forceinline__ bool gj_invert(c64 (&r)[NB], const Smem<NB>& sm, int t, int a, bool live,
                                           double theta2) {
   using G = Geo<NB>;
+  double thr = 0.0;
+#pragma unroll
+  for (int j = 0; j < NB; ++j) thr = fmax(thr, cabs2(r[j]));
+  thr *= theta2;
   bool used = false;
   bool any_search = false;
+  c64 dinv = make_double2(1.0, 0.0);
 #pragma unroll
   for (int k = 0; k < NB; ++k) {
     const int buf = k & 1;
-    c64* prow = sm.prow + ((size_t)buf * G::TPC + t) * NB;
+    c64* prow = sm.prow + ((size_t)buf * G::TPC + t) * (NB + 1);
     int bad = 0;
     if (a == k) {
-      bool accept = false;
-      if (!used) {
-        const double m = cabs2(r[k]);
-        double rm = 0.0;
-#pragma unroll
-        for (int j = 0; j < NB; ++j)
-          if (j != k) rm = fmax(rm, cabs2(r[j]));
-        accept = (m >= theta2 * rm) && (m > 0.0);
-      }
+      const double m = cabs2(r[k]);
+      const bool accept = !used && (m >= thr) && (m > 0.0);
       if (accept) {
-        const c64 inv = crcp(r[k]);
-#pragma unroll
-        for (int j = 0; j < NB; ++j) r[j] = (j == k) ? inv : cmul(r[j], inv);
+        const double rm = 1.0 / m;
+        dinv = make_double2(r[k].x * rm, -r[k].y * rm);
+        r[k] = make_double2(1.0, 0.0);
         used = true;
         if (live) {
 #pragma unroll
           for (int j = 0; j < NB; ++j) prow[j] = r[j];
+          prow[NB] = dinv;
           sm.pk[buf * G::TPC + t] = a;
           sm.perm[t * NB + k] = a;
         }
@@ -136,6 +139,7 @@ __device__ __forceinline__ bool gj_invert(c64 (&r)[NB], const Smem<NB>& sm, int 
       if (live) sm.ok[t] = accept ? 1 : 0;
       bad = (live && !accept) ? 1 : 0;
     }
+    int p = k;
     if (__syncthreads_or(bad)) {
       // rare path: every task whose candidate was rejected searches column k over its unused rows
       any_search = true;
@@ -151,28 +155,31 @@ __device__ __forceinline__ bool gj_invert(c64 (&r)[NB], const Smem<NB>& sm, int 
           if (v > bm) { bm = v; best = i; }
         }
         if (a == best) {
-          const c64 inv = crcp(r[k]);
-#pragma unroll
-          for (int j = 0; j < NB; ++j) r[j] = (j == k) ? inv : cmul(r[j], inv);
+          const double rm = 1.0 / cabs2(r[k]);
+          dinv = make_double2(r[k].x * rm, -r[k].y * rm);
+          r[k] = make_double2(1.0, 0.0);
           used = true;
           if (live) {
 #pragma unroll
             for (int j = 0; j < NB; ++j) prow[j] = r[j];
+            prow[NB] = dinv;
             sm.pk[buf * G::TPC + t] = a;
             sm.perm[t * NB + k] = a;
           }
         }
       }
       __syncthreads();
+      p = sm.pk[buf * G::TPC + t];
     }
-    const int p = sm.pk[buf * G::TPC + t];
     if (a != p) {
-      const c64 f = r[k];
+      const c64 f = cmul(r[k], prow[NB]);
       r[k] = make_double2(0.0, 0.0);
 #pragma unroll
       for (int j = 0; j < NB; ++j) cfms(r[j], f, prow[j]);
     }
   }
+#pragma unroll
+  for (int j = 0; j < NB; ++j) r[j] = cmul(r[j], dinv);
   return any_search;
 }
 

@@ -32,6 +32,8 @@ struct BlockPath {
   int* csr_rowptr;
   int* csr_col;
   double2* csr_val;
+  double2* csr_diag;
+  int diag_mask;
   int nnz_cap;
   double2* lead_mats;
   double2* table;
@@ -84,7 +86,7 @@ cudaError_t upload_vec(T** dst, const void* src, size_t count) {
 
 void block_path_destroy(BlockPath* bp) {
   if (!bp) return;
-  cudaFree(bp->csr_rowptr); cudaFree(bp->csr_col); cudaFree(bp->csr_val);
+  cudaFree(bp->csr_rowptr); cudaFree(bp->csr_col); cudaFree(bp->csr_val); cudaFree(bp->csr_diag);
   cudaFree(bp->lead_mats); cudaFree(bp->table); cudaFree(bp->hist);
   cudaFree(bp->partial); cudaFree(bp->scratch); cudaFree(bp->flags);
   delete bp;
@@ -169,6 +171,21 @@ negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, c
   chk(upload_vec(&bp->csr_rowptr, rowptr.data(), rowptr.size()));
   chk(upload_vec(&bp->csr_col, col.data(), col.size()));
   chk(upload_vec(&bp->csr_val, val.data(), val.size()));
+  {
+    std::vector<double2> dg((size_t)4 * n);
+    bp->diag_mask = 0;
+    for (int m = 0; m < 4; ++m) {
+      bool is_diag = true;
+      for (int r = 0; r < n; ++r)
+        for (int c = 0; c < n; ++c) {
+          const zc v = (*four[m])[(size_t)r * n + c];
+          if (r == c) dg[(size_t)m * n + r] = make_double2(v.real(), v.imag());
+          else if (v != zc(0, 0)) is_diag = false;
+        }
+      if (is_diag) bp->diag_mask |= 1 << m;
+    }
+    chk(upload_vec(&bp->csr_diag, dg.data(), dg.size()));
+  }
   chk(upload_vec(&bp->lead_mats, lead.data(), lead.size()));
 
   // ---- geometry and workspace plan
@@ -255,6 +272,7 @@ negf_status block_path_run(BlockPath* bp, const double* U_dev, double* n_res, do
   p.hist = bp->hist; p.partial = bp->partial; p.T = T_res;
   p.csr.rowptr = bp->csr_rowptr; p.csr.col = bp->csr_col; p.csr.val = bp->csr_val;
   p.csr.nnz_cap = bp->nnz_cap;
+  p.csr.diag = bp->csr_diag; p.csr.diag_mask = bp->diag_mask;
   for (long long begin = 0; begin < bp->total_cta; begin += bp->slots) {
     p.cta_begin = begin;
     p.n_cta = (int)std::min<long long>(bp->slots, bp->total_cta - begin);

@@ -40,6 +40,8 @@ struct CsrSet {
   const int* col;        // [4][nnz_cap]
   const double2* val;    // [4][nnz_cap]
   int nnz_cap;           // max nnz over the four
+  const double2* diag;   // [4][nb] diagonal entries of the four matrices
+  int diag_mask;         // bit m set: matrix m is diagonal (its products stay in registers)
 };
 enum { CSR_E = 0, CSR_EDAG = 1, CSR_O = 2, CSR_ODAG = 3 };
 

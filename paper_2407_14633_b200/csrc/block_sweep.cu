@@ -69,12 +69,22 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 2) block_sweep_kernel(const 
 
   // couplings of this direction, by parity of the bond: [0] even bond, [1] odd bond
   Csr Kpar[2];
+  c64* kd[2];                       // their diagonals (used when the coupling is a diagonal matrix)
+  bool kdiag[2];
   {
     const int m0 = dir ? CSR_E : CSR_EDAG, m1 = dir ? CSR_O : CSR_ODAG;
     nxt = csr_to_shared(Kpar[0], nxt, p.csr.rowptr + m0 * (NB + 1), p.csr.col + (size_t)m0 * p.csr.nnz_cap,
                         p.csr.val + (size_t)m0 * p.csr.nnz_cap, NB, p.csr.nnz_cap);
     nxt = csr_to_shared(Kpar[1], nxt, p.csr.rowptr + m1 * (NB + 1), p.csr.col + (size_t)m1 * p.csr.nnz_cap,
                         p.csr.val + (size_t)m1 * p.csr.nnz_cap, NB, p.csr.nnz_cap);
+    kd[0] = reinterpret_cast<c64*>(nxt);
+    kd[1] = kd[0] + NB;
+    if (tid < NB) {
+      kd[0][tid] = p.csr.diag[m0 * NB + tid];
+      kd[1][tid] = p.csr.diag[m1 * NB + tid];
+    }
+    kdiag[0] = (p.csr.diag_mask >> m0) & 1;
+    kdiag[1] = (p.csr.diag_mask >> m1) & 1;
   }
   __syncthreads();
 
@@ -82,9 +92,12 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 2) block_sweep_kernel(const 
   c64* hb = p.hist + (size_t)blockIdx.x * N * G::STEP_ELEMS + tid;   // + (s * NB + b) * THREADS
 
   // ------------------------------------------------------------------ connected Green's functions
-  for (int s = 0; s < N; ++s) {
+  // Loop invariant at the top of step s > 0: d = row a of ytilde_{s-1} in registers; if the coupling
+  // entering step s is not diagonal, ytilde_{s-1} is also in the task's exchange matrix.
+  c64 d[NB];
+  c64* hp = hb;
+  for (int s = 0; s < N; ++s, hp += G::STEP_ELEMS) {
     const int i = dir ? N - 1 - s : s;
-    c64 d[NB];
     if (s == 0) {
 #pragma unroll
       for (int b = 0; b < NB; ++b) {
@@ -93,10 +106,16 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 2) block_sweep_kernel(const 
       }
     } else {
       const int par = dir ? (i & 1) : ((i - 1) & 1);
-      sparse_left<NB>(d, Kpar[par], mat_t, a);                   // K_s ytilde_{s-1}
+      if (kdiag[par]) {
+        const c64 ka = kd[par][a];                                 // (K ytilde)_ab = K_aa ytilde_ab
+#pragma unroll
+        for (int b = 0; b < NB; ++b) d[b] = cmul(ka, d[b]);
+      } else {
+        sparse_left<NB>(d, Kpar[par], mat_t, a);                   // K_s ytilde_{s-1}
+      }
       if (contour) {
 #pragma unroll
-        for (int b = 0; b < NB; ++b) hb[((size_t)s * NB + b) * G::THREADS] = d[b];
+        for (int b = 0; b < NB; ++b) hp[(size_t)b * G::THREADS] = d[b];
         if (s == N - 1) break;
       }
 #pragma unroll
@@ -115,25 +134,44 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 2) block_sweep_kernel(const 
     for (int b = 0; b < NB; ++b)
       if (b == a) { d[b].x += zu; d[b].y += z.y; }
     const bool permuted = gj_invert<NB>(d, sm, t, a, live, p.theta2);
-    store_inverse<NB>(d, mat_t, sm, t, a, live, permuted);
-    __syncthreads();
+    int parn = 0;
+    bool next_diag = false;
     if (s < N - 1) {
       const int inext = dir ? i - 1 : i + 1;
-      const int par = dir ? (inext & 1) : ((inext - 1) & 1);
-      sparse_right_dagger<NB>(d, Kpar[par], mat_t + a * NB);     // ytilde_s = g_s K_{s+1}^dagger
+      parn = dir ? (inext & 1) : ((inext - 1) & 1);
+      next_diag = kdiag[parn];
+    }
+    if (s == N - 1 || next_diag) {
+      if (permuted) {                                              // rare: undo the implicit row order
+        store_inverse<NB>(d, mat_t, sm, t, a, live, true);
+        __syncthreads();
+#pragma unroll
+        for (int b = 0; b < NB; ++b) d[b] = mat_t[a * NB + b];
+      }
+      if (s < N - 1) {
+        const c64* kdn = kd[parn];                                 // ytilde_ab = g_ab conj(K_bb)
+#pragma unroll
+        for (int b = 0; b < NB; ++b) d[b] = cmul(d[b], cconj(kdn[b]));
+      }                                                            // last ring: G_(k,k) itself
+      if (!contour) {
+#pragma unroll
+        for (int b = 0; b < NB; ++b) hp[(size_t)b * G::THREADS] = d[b];
+      }
+      __syncthreads();                                             // separates consecutive gj_invert calls
     } else {
+      store_inverse<NB>(d, mat_t, sm, t, a, live, permuted);
+      __syncthreads();
+      sparse_right_dagger<NB>(d, Kpar[parn], mat_t + a * NB);      // ytilde_s = g_s K_{s+1}^dagger
+      if (!contour) {
 #pragma unroll
-      for (int b = 0; b < NB; ++b) d[b] = mat_t[a * NB + b];      // last ring: G_(k,k) itself
-    }
-    if (!contour) {
+        for (int b = 0; b < NB; ++b) hp[(size_t)b * G::THREADS] = d[b];
+      }
+      if (live) {                                                  // only this thread reads row a above
 #pragma unroll
-      for (int b = 0; b < NB; ++b) hb[((size_t)s * NB + b) * G::THREADS] = d[b];
+        for (int b = 0; b < NB; ++b) mat_t[a * NB + b] = d[b];
+      }
+      __syncthreads();
     }
-    if (live) {
-#pragma unroll
-      for (int b = 0; b < NB; ++b) mat_t[a * NB + b] = d[b];
-    }
-    __syncthreads();
   }
   if (contour) return;
 
@@ -292,7 +330,7 @@ block_combine_kernel(const SweepLaunch p, long long pair_cta_begin, int rings_pe
 
 template <int NB>
 static size_t sweep_smem_t(int nnz_cap) {
-  return Smem<NB>::bytes(1) + 2 * csr_shared_bytes(NB, nnz_cap) + 32;
+  return Smem<NB>::bytes(1) + 2 * csr_shared_bytes(NB, nnz_cap) + 2 * NB * sizeof(c64) + 32;
 }
 
 template <int NB>
