@@ -219,14 +219,14 @@ negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, c
     return fail(NEGF_ECUDA);
   }
   bp->wave = std::max(2, bp->ctas_per_sm * sms);
-  bp->slot_bytes = (int64_t)sizeof(double2) * bp->N * n * bp->threads;
+  bp->slot_bytes = (int64_t)sizeof(double2) * bp->N * blk::block_step_elems(n);
   size_t free_b = 0, total_b = 0;
   cudaMemGetInfo(&free_b, &total_b);
   int64_t budget = cfg->workspace_bytes > 0 ? cfg->workspace_bytes : (int64_t)((double)free_b * 0.85);
   budget = std::min<int64_t>(budget, (int64_t)((double)free_b * 0.95));
   long long slots = std::min<long long>(bp->total_cta, budget / bp->slot_bytes);
   slots = std::min<long long>(slots, 2LL * bp->wave);
-  if (slots > bp->wave) slots = slots / bp->wave * bp->wave;
+  if (slots > bp->wave && slots < bp->total_cta) slots = slots / bp->wave * bp->wave;
   slots &= ~1LL;
   if (slots < 2) {
     set_error("negf_create: recursion-history workspace too small (need >= %lld bytes for two CTAs)",

@@ -76,7 +76,7 @@ struct SweepLaunch {
   const double2* table;       // Sigma / F table of SrLaunch
   double mu_s, mu_d, kT, deg;
   double theta2;              // pivot acceptance threshold (block_ops.cuh)
-  double2* hist;              // [slots][N][nb][THREADS]
+  double2* hist;              // [slots][N][2 row slots][nb][THREADS]
   double* partial;            // [C][geq + 2 gneq][N]
   double* T;                  // [C][K_neq]
   CsrSet csr;
@@ -89,6 +89,7 @@ cudaError_t launch_block_combine(int nb, const SweepLaunch& p, long long pair_ct
 // Geometry queries (host).
 int block_tasks_per_cta(int nb);
 int block_threads(int nb);
+long long block_step_elems(int nb);   // history elements per ring step per CTA
 size_t block_sweep_smem(int nb, int nnz_cap);
 int block_sweep_ctas_per_sm(int nb, int nnz_cap);
 bool block_size_supported(int nb);

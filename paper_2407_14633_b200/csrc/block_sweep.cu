@@ -12,7 +12,7 @@
 //     Tr A_k,(i,i) = ||C_s||_F^2,   T = ||F_first^dagger C_0||_F^2   (eq.(5))
 // Contour points need Tr G_(i,i) = Tr [alpha_i - x_i - y_i]^-1 (Alg.1 step 1): their two half-sweeps
 // store x_i / y_i = K_s ytilde_{s-1} and a second kernel (parallel over rings) inverts and traces.
-#include "block_ops.cuh"
+#include "block_ops2.cuh"
 #include "block_path.h"
 #include "negf_internal.h"
 
@@ -38,16 +38,84 @@ __device__ __forceinline__ CtaId decode_cta(const SweepLaunch& p, long long gid)
   return id;
 }
 
+// Explicit shared-memory loads (32-bit shared addresses): the CSR tables are reached through
+// pointers selected at run time, for which the compiler otherwise falls back to generic loads.
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ int lds_i32(unsigned addr) {
+  int v;
+  asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ c64 lds_c64(unsigned addr) {
+  c64 v;
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+  return v;
+}
+struct CsrS {            // CSR matrix in shared memory, by shared address
+  unsigned rowptr, col, val;
+};
+__device__ __forceinline__ CsrS csr_shared(const Csr& K) {
+  return CsrS{smem_addr(K.rowptr), smem_addr(K.col), smem_addr(K.val)};
+}
+
+// y[q][b] = sum_{c in nz(K_rid)} K[rid][c] * X[c][b] for the thread's two rows (X in shared memory)
 template <int NB>
-__global__ void __launch_bounds__(Geo<NB>::THREADS, 2) block_sweep_kernel(const SweepLaunch p) {
-  using G = Geo<NB>;
+__device__ __forceinline__ void sparse_left2(c64 (&y)[2][NB], const CsrS K, unsigned X, int a, bool valid1) {
+  constexpr int TPT = Geo2<NB>::TPT;
+#pragma unroll
+  for (int q = 0; q < 2; ++q) {
+#pragma unroll
+    for (int b = 0; b < NB; ++b) y[q][b] = make_double2(0.0, 0.0);
+    if (q == 1 && !valid1) continue;
+    const int rid = a + q * TPT;
+    const int e0 = lds_i32(K.rowptr + 4 * rid), e1 = lds_i32(K.rowptr + 4 * rid + 4);
+#pragma unroll 1
+    for (int e = e0; e < e1; ++e) {
+      const c64 v = lds_c64(K.val + 16 * e);
+      const unsigned xr = X + (unsigned)lds_i32(K.col + 4 * e) * (NB * 16);
+#pragma unroll
+      for (int b = 0; b < NB; ++b) cfma(y[q][b], v, lds_c64(xr + 16 * b));
+    }
+  }
+}
+
+// y[q][b] = sum_{d in nz(K_b)} X[rid][d] * conj(K[b][d])   (rows of X K^dagger from the thread's own rows
+// of X in shared memory)
+template <int NB>
+__device__ __forceinline__ void sparse_right_dagger2(c64 (&y)[2][NB], const CsrS K, unsigned X, int a,
+                                                     bool valid1) {
+  constexpr int TPT = Geo2<NB>::TPT;
+  const unsigned x0 = X + a * (NB * 16);
+  const unsigned x1 = X + (valid1 ? a + TPT : a) * (NB * 16);
+#pragma unroll
+  for (int b = 0; b < NB; ++b) {
+    c64 acc0 = make_double2(0.0, 0.0), acc1 = make_double2(0.0, 0.0);
+    const int e0 = lds_i32(K.rowptr + 4 * b), e1 = lds_i32(K.rowptr + 4 * b + 4);
+#pragma unroll 1
+    for (int e = e0; e < e1; ++e) {
+      const c64 kv = cconj(lds_c64(K.val + 16 * e));
+      const unsigned cidx = 16u * (unsigned)lds_i32(K.col + 4 * e);
+      cfma(acc0, lds_c64(x0 + cidx), kv);
+      cfma(acc1, lds_c64(x1 + cidx), kv);
+    }
+    y[0][b] = acc0;
+    y[1][b] = valid1 ? acc1 : make_double2(0.0, 0.0);
+  }
+}
+
+template <int NB>
+__global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_sweep_kernel(const SweepLaunch p) {
+  using G = Geo2<NB>;
+  constexpr int TPT = G::TPT;
   extern __shared__ __align__(16) char smem_raw[];
-  Smem<NB> sm;
-  char* nxt = sm.carve(smem_raw, 1);
+  Smem2<NB> sm;
+  char* nxt = sm.carve(smem_raw);
   const int tid = threadIdx.x;
   const bool live = tid < G::LIVE;
-  const int t = live ? tid / NB : 0;
-  const int a = tid % NB;
+  const int t = live ? tid / TPT : 0;
+  const int a = tid % TPT;
+  const bool valid1 = a + TPT < NB;
+  const int rid1 = valid1 ? a + TPT : a;            // clamped row index for address computations
   const int lane = tid & 31, warp = tid >> 5;
   const int N = p.N;
 
@@ -68,20 +136,23 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 2) block_sweep_kernel(const 
   const double* Uc = p.U + (size_t)id.c * N;
 
   // couplings of this direction, by parity of the bond: [0] even bond, [1] odd bond
-  Csr Kpar[2];
+  Csr Kgen[2];
+  CsrS Kpar[2];
   c64* kd[2];                       // their diagonals (used when the coupling is a diagonal matrix)
   bool kdiag[2];
   {
     const int m0 = dir ? CSR_E : CSR_EDAG, m1 = dir ? CSR_O : CSR_ODAG;
-    nxt = csr_to_shared(Kpar[0], nxt, p.csr.rowptr + m0 * (NB + 1), p.csr.col + (size_t)m0 * p.csr.nnz_cap,
+    nxt = csr_to_shared(Kgen[0], nxt, p.csr.rowptr + m0 * (NB + 1), p.csr.col + (size_t)m0 * p.csr.nnz_cap,
                         p.csr.val + (size_t)m0 * p.csr.nnz_cap, NB, p.csr.nnz_cap);
-    nxt = csr_to_shared(Kpar[1], nxt, p.csr.rowptr + m1 * (NB + 1), p.csr.col + (size_t)m1 * p.csr.nnz_cap,
+    nxt = csr_to_shared(Kgen[1], nxt, p.csr.rowptr + m1 * (NB + 1), p.csr.col + (size_t)m1 * p.csr.nnz_cap,
                         p.csr.val + (size_t)m1 * p.csr.nnz_cap, NB, p.csr.nnz_cap);
+    Kpar[0] = csr_shared(Kgen[0]);
+    Kpar[1] = csr_shared(Kgen[1]);
     kd[0] = reinterpret_cast<c64*>(nxt);
     kd[1] = kd[0] + NB;
-    if (tid < NB) {
-      kd[0][tid] = p.csr.diag[m0 * NB + tid];
-      kd[1][tid] = p.csr.diag[m1 * NB + tid];
+    for (int i = tid; i < NB; i += G::THREADS) {
+      kd[0][i] = p.csr.diag[m0 * NB + i];
+      kd[1][i] = p.csr.diag[m1 * NB + i];
     }
     kdiag[0] = (p.csr.diag_mask >> m0) & 1;
     kdiag[1] = (p.csr.diag_mask >> m1) & 1;
@@ -89,51 +160,68 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 2) block_sweep_kernel(const 
   __syncthreads();
 
   c64* mat_t = sm.mat + (size_t)t * G::MAT;
-  c64* hb = p.hist + (size_t)blockIdx.x * N * G::STEP_ELEMS + tid;   // + (s * NB + b) * THREADS
+  const unsigned mat_s = smem_addr(mat_t);
+  c64* hb = p.hist + (size_t)blockIdx.x * N * G::STEP_ELEMS + tid;   // + ((s*2 + q)*NB + b) * THREADS
+  constexpr size_t HQ = (size_t)NB * G::THREADS;                     // offset of the second row slot
 
   // ------------------------------------------------------------------ connected Green's functions
-  // Loop invariant at the top of step s > 0: d = row a of ytilde_{s-1} in registers; if the coupling
+  // Loop invariant at the top of step s > 0: d = the thread's rows of ytilde_{s-1}; if the coupling
   // entering step s is not diagonal, ytilde_{s-1} is also in the task's exchange matrix.
-  c64 d[NB];
+  c64 d[2][NB];
   c64* hp = hb;
   for (int s = 0; s < N; ++s, hp += G::STEP_ELEMS) {
     const int i = dir ? N - 1 - s : s;
     if (s == 0) {
 #pragma unroll
       for (int b = 0; b < NB; ++b) {
-        const c64 sg = tab_first[a * NB + b];
-        d[b] = make_double2(-sg.x, -sg.y);
+        const c64 s0 = tab_first[a * NB + b], s1 = tab_first[rid1 * NB + b];
+        d[0][b] = make_double2(-s0.x, -s0.y);
+        d[1][b] = valid1 ? make_double2(-s1.x, -s1.y) : make_double2(0.0, 0.0);
       }
     } else {
       const int par = dir ? (i & 1) : ((i - 1) & 1);
       if (kdiag[par]) {
-        const c64 ka = kd[par][a];                                 // (K ytilde)_ab = K_aa ytilde_ab
+        const c64 k0 = kd[par][a], k1 = kd[par][rid1];             // (K ytilde)_ab = K_aa ytilde_ab
 #pragma unroll
-        for (int b = 0; b < NB; ++b) d[b] = cmul(ka, d[b]);
+        for (int b = 0; b < NB; ++b) {
+          d[0][b] = cmul(k0, d[0][b]);
+          d[1][b] = cmul(k1, d[1][b]);
+        }
       } else {
-        sparse_left<NB>(d, Kpar[par], mat_t, a);                   // K_s ytilde_{s-1}
+        sparse_left2<NB>(d, Kpar[par], mat_s, a, valid1);          // K_s ytilde_{s-1}
       }
       if (contour) {
+        if (live) {
 #pragma unroll
-        for (int b = 0; b < NB; ++b) hp[(size_t)b * G::THREADS] = d[b];
+          for (int b = 0; b < NB; ++b) {
+            hp[(size_t)b * G::THREADS] = d[0][b];
+            if (valid1) hp[HQ + (size_t)b * G::THREADS] = d[1][b];
+          }
+        }
         if (s == N - 1) break;
       }
 #pragma unroll
-      for (int b = 0; b < NB; ++b) d[b] = make_double2(-d[b].x, -d[b].y);
+      for (int b = 0; b < NB; ++b) {
+        d[0][b] = make_double2(-d[0][b].x, -d[0][b].y);
+        d[1][b] = make_double2(-d[1][b].x, -d[1][b].y);
+      }
     }
     if (!contour && s == N - 1) {
 #pragma unroll
       for (int b = 0; b < NB; ++b) {
-        const c64 sg = tab_last[a * NB + b];
-        d[b].x -= sg.x;
-        d[b].y -= sg.y;
+        const c64 s0 = tab_last[a * NB + b], s1 = tab_last[rid1 * NB + b];
+        d[0][b].x -= s0.x;
+        d[0][b].y -= s0.y;
+        if (valid1) { d[1][b].x -= s1.x; d[1][b].y -= s1.y; }
       }
     }
     const double zu = z.x - Uc[i];
 #pragma unroll
-    for (int b = 0; b < NB; ++b)
-      if (b == a) { d[b].x += zu; d[b].y += z.y; }
-    const bool permuted = gj_invert<NB>(d, sm, t, a, live, p.theta2);
+    for (int b = 0; b < NB; ++b) {
+      if (b == a) { d[0][b].x += zu; d[0][b].y += z.y; }
+      if (b == a + TPT) { d[1][b].x += zu; d[1][b].y += z.y; }
+    }
+    const bool permuted = gj_invert2<NB>(d, sm, t, a, live, p.theta2);
     int parn = 0;
     bool next_diag = false;
     if (s < N - 1) {
@@ -143,32 +231,45 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 2) block_sweep_kernel(const 
     }
     if (s == N - 1 || next_diag) {
       if (permuted) {                                              // rare: undo the implicit row order
-        store_inverse<NB>(d, mat_t, sm, t, a, live, true);
+        store_inverse2<NB>(d, mat_t, sm, t, a, live, true);
         __syncthreads();
 #pragma unroll
-        for (int b = 0; b < NB; ++b) d[b] = mat_t[a * NB + b];
+        for (int b = 0; b < NB; ++b) {
+          d[0][b] = mat_t[a * NB + b];
+          d[1][b] = valid1 ? mat_t[rid1 * NB + b] : make_double2(0.0, 0.0);
+        }
       }
       if (s < N - 1) {
         const c64* kdn = kd[parn];                                 // ytilde_ab = g_ab conj(K_bb)
 #pragma unroll
-        for (int b = 0; b < NB; ++b) d[b] = cmul(d[b], cconj(kdn[b]));
+        for (int b = 0; b < NB; ++b) {
+          const c64 kb = cconj(kdn[b]);
+          d[0][b] = cmul(d[0][b], kb);
+          d[1][b] = cmul(d[1][b], kb);
+        }
       }                                                            // last ring: G_(k,k) itself
-      if (!contour) {
+      if (!contour && live) {
 #pragma unroll
-        for (int b = 0; b < NB; ++b) hp[(size_t)b * G::THREADS] = d[b];
+        for (int b = 0; b < NB; ++b) {
+          hp[(size_t)b * G::THREADS] = d[0][b];
+          if (valid1) hp[HQ + (size_t)b * G::THREADS] = d[1][b];
+        }
       }
-      __syncthreads();                                             // separates consecutive gj_invert calls
+      __syncthreads();                                             // separates consecutive gj_invert2 calls
     } else {
-      store_inverse<NB>(d, mat_t, sm, t, a, live, permuted);
+      store_inverse2<NB>(d, mat_t, sm, t, a, live, permuted);
       __syncthreads();
-      sparse_right_dagger<NB>(d, Kpar[parn], mat_t + a * NB);      // ytilde_s = g_s K_{s+1}^dagger
-      if (!contour) {
+      sparse_right_dagger2<NB>(d, Kpar[parn], mat_s, a, valid1);   // ytilde_s = g_s K_{s+1}^dagger
+      if (live) {
 #pragma unroll
-        for (int b = 0; b < NB; ++b) hp[(size_t)b * G::THREADS] = d[b];
-      }
-      if (live) {                                                  // only this thread reads row a above
-#pragma unroll
-        for (int b = 0; b < NB; ++b) mat_t[a * NB + b] = d[b];
+        for (int b = 0; b < NB; ++b) {
+          if (!contour) hp[(size_t)b * G::THREADS] = d[0][b];
+          mat_t[a * NB + b] = d[0][b];
+          if (valid1) {
+            if (!contour) hp[HQ + (size_t)b * G::THREADS] = d[1][b];
+            mat_t[rid1 * NB + b] = d[1][b];
+          }
+        }
       }
       __syncthreads();
     }
@@ -184,29 +285,62 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 2) block_sweep_kernel(const 
     const c64* F_last = tab_last + G::MAT;
     if (live) {
 #pragma unroll
-      for (int b = 0; b < NB; ++b) mat_t[a * NB + b] = F_last[a * NB + b];
+      for (int b = 0; b < NB; ++b) {
+        mat_t[a * NB + b] = F_last[a * NB + b];
+        if (valid1) mat_t[rid1 * NB + b] = F_last[rid1 * NB + b];
+      }
     }
   }
-  c64 A[NB];
-#pragma unroll
-  for (int kq = 0; kq < NB; ++kq) A[kq] = hb[((size_t)(N - 1) * NB + kq) * G::THREADS];
+  // The thread's two rows of ytilde_s stream through registers one column at a time.  Three register
+  // pairs P[0..2] hold columns 3g, 3g+1, 3g+2 of the current group; each is refilled, right after its
+  // use, with the column three slots ahead (a ring is padded to NG*3 slots so that the slot -> register
+  // assignment is static; the loop over groups is not unrolled: instruction-cache footprint).
+  constexpr int NG = (NB + 2) / 3;
+  const c64* pf = hb + (size_t)(N - 1) * G::STEP_ELEMS;   // prefetch cursor: ring pf_ring, slot pf_kq
+  int pf_ring = N - 1, pf_kq = 0;
+  c64 P[3][2];
+  auto fetch = [&](c64 (&dst)[2]) {
+    if (pf_kq < NB) {
+      dst[0] = pf[0];
+      dst[1] = valid1 ? pf[HQ] : make_double2(0.0, 0.0);
+    }
+    pf += G::THREADS;
+    if (++pf_kq == 3 * NG) {
+      pf_kq = 0;
+      pf -= (size_t)3 * NG * G::THREADS;
+      if (pf_ring > 0) { --pf_ring; pf -= G::STEP_ELEMS; }
+    }
+  };
+  fetch(P[0]);
+  fetch(P[1]);
+  fetch(P[2]);
   __syncthreads();
-  c64 cc[NB];
+  c64 cc[2][NB];
   for (int s = N - 1; s >= 0; --s) {
     const int i = dir ? N - 1 - s : s;
-    const c64* hnext = hb + (size_t)(s > 0 ? s - 1 : 0) * NB * G::THREADS;
 #pragma unroll
-    for (int b = 0; b < NB; ++b) cc[b] = make_double2(0.0, 0.0);
+    for (int b = 0; b < NB; ++b) cc[0][b] = cc[1][b] = make_double2(0.0, 0.0);
+#pragma unroll 1
+    for (int g = 0; g < NG; ++g) {
 #pragma unroll
-    for (int kq = 0; kq < NB; ++kq) {
-      const c64 av = A[kq];
-      A[kq] = hnext[(size_t)kq * G::THREADS];                     // prefetch ring s-1 of the history
+      for (int u = 0; u < 3; ++u) {
+        const int kq = 3 * g + u;
+        const c64 av0 = P[u][0], av1 = P[u][1];
+        fetch(P[u]);
+        if (kq < NB) {
+          const c64* brow = mat_t + kq * NB;
 #pragma unroll
-      for (int b = 0; b < NB; ++b) cfma(cc[b], av, mat_t[kq * NB + b]);
+          for (int b = 0; b < NB; ++b) {
+            const c64 bv = brow[b];
+            cfma(cc[0][b], av0, bv);
+            cfma(cc[1][b], av1, bv);
+          }
+        }
+      }
     }
     double v = 0.0;
 #pragma unroll
-    for (int b = 0; b < NB; ++b) v += cabs2(cc[b]);
+    for (int b = 0; b < NB; ++b) v += cabs2(cc[0][b]) + cabs2(cc[1][b]);
     v = live ? wt * v : 0.0;
     v = warp_sum(v);
     if (lane == 0) sm.red[(s & 1) * G::NWARPS + warp] = v;
@@ -220,7 +354,10 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 2) block_sweep_kernel(const 
     if (s > 0) {
       if (live) {
 #pragma unroll
-        for (int b = 0; b < NB; ++b) mat_t[a * NB + b] = cc[b];
+        for (int b = 0; b < NB; ++b) {
+          mat_t[a * NB + b] = cc[0][b];
+          if (valid1) mat_t[rid1 * NB + b] = cc[1][b];
+        }
       }
       __syncthreads();
     }
@@ -230,24 +367,32 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 2) block_sweep_kernel(const 
     const c64* F_first = tab_first + G::MAT;
     if (live) {
 #pragma unroll
-      for (int b = 0; b < NB; ++b) mat_t[a * NB + b] = cc[b];      // C_0 = G_(0,N-1) F_R
+      for (int b = 0; b < NB; ++b) {                               // C_0 = G_(0,N-1) F_R
+        mat_t[a * NB + b] = cc[0][b];
+        if (valid1) mat_t[rid1 * NB + b] = cc[1][b];
+      }
     }
     __syncthreads();
 #pragma unroll
-    for (int b = 0; b < NB; ++b) cc[b] = make_double2(0.0, 0.0);
-    for (int c2 = 0; c2 < NB; ++c2) {
-      const c64 f = cconj(F_first[c2 * NB + a]);
+    for (int b = 0; b < NB; ++b) cc[0][b] = cc[1][b] = make_double2(0.0, 0.0);
+    for (int c2 = 0; c2 < NB; ++c2) {                              // rows of F_first^dagger C_0
+      const c64 f0 = cconj(F_first[c2 * NB + a]);
+      const c64 f1 = valid1 ? cconj(F_first[c2 * NB + rid1]) : make_double2(0.0, 0.0);
 #pragma unroll
-      for (int b = 0; b < NB; ++b) cfma(cc[b], f, mat_t[c2 * NB + b]);
+      for (int b = 0; b < NB; ++b) {
+        const c64 bv = mat_t[c2 * NB + b];
+        cfma(cc[0][b], f0, bv);
+        cfma(cc[1][b], f1, bv);
+      }
     }
     double v = 0.0;
 #pragma unroll
-    for (int b = 0; b < NB; ++b) v += cabs2(cc[b]);
+    for (int b = 0; b < NB; ++b) v += cabs2(cc[0][b]) + cabs2(cc[1][b]);
     if (live) sm.mag[t * NB + a] = v;
     __syncthreads();
     if (a == 0 && active) {
       double tot = 0.0;
-      for (int r = 0; r < NB; ++r) tot += sm.mag[t * NB + r];
+      for (int r = 0; r < TPT; ++r) tot += sm.mag[t * NB + r];
       p.T[(size_t)id.c * p.K_neq + k] = tot;
     }
   }
@@ -256,16 +401,19 @@ __global__ void __launch_bounds__(Geo<NB>::THREADS, 2) block_sweep_kernel(const 
 // Contour combine: G_(i,i) = [alpha_i - x_i - y_i]^-1 (Alg.1 step 1) and the first term
 // of eq.(4): -(deg/pi) Im[W_k Tr G_(i,i)].  grid = (ring chunks, pairs of contour sweep CTAs).
 template <int NB>
-__global__ void __launch_bounds__(Geo<NB>::THREADS, 2)
+__global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1))
 block_combine_kernel(const SweepLaunch p, long long pair_cta_begin, int rings_per_cta) {
-  using G = Geo<NB>;
+  using G = Geo2<NB>;
+  constexpr int TPT = G::TPT;
   extern __shared__ __align__(16) char smem_raw[];
-  Smem<NB> sm;
-  sm.carve(smem_raw, 1);
+  Smem2<NB> sm;
+  sm.carve(smem_raw);
   const int tid = threadIdx.x;
   const bool live = tid < G::LIVE;
-  const int t = live ? tid / NB : 0;
-  const int a = tid % NB;
+  const int t = live ? tid / TPT : 0;
+  const int a = tid % TPT;
+  const bool valid1 = a + TPT < NB;
+  const int rid1 = valid1 ? a + TPT : a;
   const int lane = tid & 31, warp = tid >> 5;
   const int N = p.N;
   const long long gid = pair_cta_begin + 2 * (long long)blockIdx.y;
@@ -283,6 +431,7 @@ block_combine_kernel(const SweepLaunch p, long long pair_cta_begin, int rings_pe
   const double* Uc = p.U + (size_t)id.c * N;
   const c64* hL = p.hist + slotL * N * G::STEP_ELEMS + tid;
   const c64* hR = p.hist + (slotL + 1) * N * G::STEP_ELEMS + tid;
+  constexpr size_t HQ = (size_t)NB * G::THREADS;
   c64* mat_t = sm.mat + (size_t)t * G::MAT;
   const int R = p.geq + 2 * p.gneq;
   double* prow_out = p.partial + ((size_t)id.c * R + id.grp) * N;
@@ -290,27 +439,41 @@ block_combine_kernel(const SweepLaunch p, long long pair_cta_begin, int rings_pe
   const int i0 = blockIdx.x * rings_per_cta;
   const int i1 = min(N, i0 + rings_per_cta);
   for (int i = i0; i < i1; ++i) {
-    c64 d[NB];
+    c64 d[2][NB];
+    const c64* pl = hL + (size_t)i * G::STEP_ELEMS;
+    const c64* pr = hR + (size_t)(N - 1 - i) * G::STEP_ELEMS;
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
-      const c64 yl = (i == 0) ? tabL[a * NB + b] : hL[((size_t)i * NB + b) * G::THREADS];
-      const c64 xr = (i == N - 1) ? tabR[a * NB + b] : hR[((size_t)(N - 1 - i) * NB + b) * G::THREADS];
-      d[b] = make_double2(-yl.x - xr.x, -yl.y - xr.y);
+      const c64 yl0 = (i == 0) ? tabL[a * NB + b] : pl[(size_t)b * G::THREADS];
+      const c64 xr0 = (i == N - 1) ? tabR[a * NB + b] : pr[(size_t)b * G::THREADS];
+      d[0][b] = make_double2(-yl0.x - xr0.x, -yl0.y - xr0.y);
+      if (valid1) {
+        const c64 yl1 = (i == 0) ? tabL[rid1 * NB + b] : pl[HQ + (size_t)b * G::THREADS];
+        const c64 xr1 = (i == N - 1) ? tabR[rid1 * NB + b] : pr[HQ + (size_t)b * G::THREADS];
+        d[1][b] = make_double2(-yl1.x - xr1.x, -yl1.y - xr1.y);
+      } else {
+        d[1][b] = make_double2(0.0, 0.0);
+      }
     }
     const double zu = z.x - Uc[i];
 #pragma unroll
-    for (int b = 0; b < NB; ++b)
-      if (b == a) { d[b].x += zu; d[b].y += z.y; }
-    const bool permuted = gj_invert<NB>(d, sm, t, a, live, p.theta2);
+    for (int b = 0; b < NB; ++b) {
+      if (b == a) { d[0][b].x += zu; d[0][b].y += z.y; }
+      if (b == a + TPT) { d[1][b].x += zu; d[1][b].y += z.y; }
+    }
+    const bool permuted = gj_invert2<NB>(d, sm, t, a, live, p.theta2);
     c64 gaa = make_double2(0.0, 0.0);
     if (!permuted) {
 #pragma unroll
-      for (int b = 0; b < NB; ++b)
-        if (b == a) gaa = d[b];
+      for (int b = 0; b < NB; ++b) {
+        if (b == a) { gaa.x += d[0][b].x; gaa.y += d[0][b].y; }
+        if (b == a + TPT) { gaa.x += d[1][b].x; gaa.y += d[1][b].y; }
+      }
     } else {
-      store_inverse<NB>(d, mat_t, sm, t, a, live, true);
+      store_inverse2<NB>(d, mat_t, sm, t, a, live, true);
       __syncthreads();
       gaa = mat_t[a * NB + a];
+      if (valid1) { gaa.x += mat_t[rid1 * NB + rid1].x; gaa.y += mat_t[rid1 * NB + rid1].y; }
     }
     double v = live ? wc * (W.x * gaa.y + W.y * gaa.x) : 0.0;
     v = warp_sum(v);
@@ -330,12 +493,12 @@ block_combine_kernel(const SweepLaunch p, long long pair_cta_begin, int rings_pe
 
 template <int NB>
 static size_t sweep_smem_t(int nnz_cap) {
-  return Smem<NB>::bytes(1) + 2 * csr_shared_bytes(NB, nnz_cap) + 2 * NB * sizeof(c64) + 32;
+  return Smem2<NB>::bytes() + 2 * csr_shared_bytes(NB, nnz_cap) + 2 * NB * sizeof(c64) + 32;
 }
 
 template <int NB>
 static cudaError_t launch_sweep_t(const SweepLaunch& p, cudaStream_t s) {
-  using G = Geo<NB>;
+  using G = Geo2<NB>;
   const size_t smem = sweep_smem_t<NB>(p.csr.nnz_cap);
   cudaError_t e = cudaFuncSetAttribute(block_sweep_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
@@ -345,8 +508,8 @@ static cudaError_t launch_sweep_t(const SweepLaunch& p, cudaStream_t s) {
 
 template <int NB>
 static cudaError_t launch_combine_t(const SweepLaunch& p, long long pair_cta_begin, int n_pairs, cudaStream_t s) {
-  using G = Geo<NB>;
-  const size_t smem = Smem<NB>::bytes(1);
+  using G = Geo2<NB>;
+  const size_t smem = Smem2<NB>::bytes();
   cudaError_t e = cudaFuncSetAttribute(block_combine_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   const int rings_per_cta = 8;
@@ -367,7 +530,7 @@ static int ctas_per_sm_t(int nnz_cap) {
   if (cudaFuncSetAttribute(block_sweep_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
       cudaSuccess)
     return 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, block_sweep_kernel<NB>, Geo<NB>::THREADS, smem) !=
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, block_sweep_kernel<NB>, Geo2<NB>::THREADS, smem) !=
       cudaSuccess)
     return 0;
   return nb;
@@ -392,7 +555,7 @@ cudaError_t launch_block_combine(int nb, const SweepLaunch& p, long long pair_ct
 }
 int block_tasks_per_cta(int nb) {
   switch (nb) {
-#define NEGF_CASE(NB_) case NB_: return Geo<NB_>::TPC;
+#define NEGF_CASE(NB_) case NB_: return Geo2<NB_>::TPC;
     NEGF_BLOCK_SIZES(NEGF_CASE)
 #undef NEGF_CASE
     default: return 0;
@@ -400,7 +563,7 @@ int block_tasks_per_cta(int nb) {
 }
 int block_threads(int nb) {
   switch (nb) {
-#define NEGF_CASE(NB_) case NB_: return Geo<NB_>::THREADS;
+#define NEGF_CASE(NB_) case NB_: return Geo2<NB_>::THREADS;
     NEGF_BLOCK_SIZES(NEGF_CASE)
 #undef NEGF_CASE
     default: return 0;
@@ -417,6 +580,14 @@ size_t block_sweep_smem(int nb, int nnz_cap) {
 int block_sweep_ctas_per_sm(int nb, int nnz_cap) {
   switch (nb) {
 #define NEGF_CASE(NB_) case NB_: return ctas_per_sm_t<NB_>(nnz_cap);
+    NEGF_BLOCK_SIZES(NEGF_CASE)
+#undef NEGF_CASE
+    default: return 0;
+  }
+}
+long long block_step_elems(int nb) {
+  switch (nb) {
+#define NEGF_CASE(NB_) case NB_: return Geo2<NB_>::STEP_ELEMS;
     NEGF_BLOCK_SIZES(NEGF_CASE)
 #undef NEGF_CASE
     default: return 0;
