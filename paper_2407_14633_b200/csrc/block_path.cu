@@ -19,7 +19,7 @@ typedef std::complex<double> zc;
 
 struct BlockPath {
   int C, N, n, K_eq, K_neq;
-  double mu_s, mu_d, kT, deg, sr_tol;
+  double mu_s, mu_d, kT, deg, sr_tol, sr_shift;
   int sr_maxit;
   const double2 *z_eq, *w_eq, *z_neq;   // owned by the negf_handle
   const double* w_neq;
@@ -117,6 +117,11 @@ negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, c
   for (size_t i = 0; i < nn; ++i) {
     E[i] = zc(cfg->coup_even[i].re, cfg->coup_even[i].im);
     O[i] = zc(cfg->coup_odd[i].re, cfg->coup_odd[i].im);
+  }
+  {
+    double vmax = 0.0;
+    for (size_t i = 0; i < nn; ++i) vmax = std::max(vmax, std::max(std::abs(E[i]), std::abs(O[i])));
+    bp->sr_shift = 1e-4 * vmax;
   }
   const std::vector<zc> Ed = mat_dag(E, n), Od = mat_dag(O, n);
   const std::vector<zc>* four[4] = {&E, &Ed, &O, &Od};     // CSR_E, CSR_EDAG, CSR_O, CSR_ODAG
@@ -251,7 +256,7 @@ negf_status block_path_self_energy(BlockPath* bp, const double* U_dev, cudaStrea
   p.C = bp->C; p.N = bp->N; p.K_eq = bp->K_eq; p.K_neq = bp->K_neq;
   p.U = U_dev; p.z_eq = bp->z_eq; p.z_neq = bp->z_neq;
   p.lead_mats = bp->lead_mats; p.table = bp->table;
-  p.tol = bp->sr_tol; p.maxit = bp->sr_maxit; p.theta2 = g_theta2;
+  p.tol = bp->sr_tol; p.shift = bp->sr_shift; p.maxit = bp->sr_maxit; p.theta2 = g_theta2;
   p.max_iters = bp->flags; p.noconv_flag = bp->flags + 1;
   NEGF_CUDA_TRY(cudaMemsetAsync(bp->flags, 0, 2 * sizeof(int), s));
   hook.begin(hook.ctx, 0);

@@ -55,6 +55,7 @@ struct SrLaunch {
                               //   L, R, V0, V1, V0^+, V1^+
   double2* table;             // [C][K_eq + K_neq][2 leads][2: Sigma, F][nb*nb]
   double tol;
+  double shift;               // imaginary energy shift of the fallback decimation (sancho_rubio.cu)
   double theta2;              // pivot acceptance threshold (block_ops.cuh)
   int maxit;
   int* max_iters;             // device scalar, atomicMax

@@ -34,6 +34,7 @@ namespace negf {
 namespace blk {
 
 constexpr int kNewtonMax = 4;
+constexpr int kDoublingMax = 64;   // 2^64 terms of the Neumann series: beyond any 1/eta
 
 // c[b] = sum_k arow[k] * X[k * LD + b]
 template <int NB, int LD>
@@ -110,7 +111,7 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
   const c64* my_init = (h == 0 ? gV1d : gV1) + a * NB;
 
   // row r of z - eps:  half 0: [z - eps_00 | -V0],  half 1: [-V0^+ | z - eps_11]
-  auto build_row = [&](c64 (&m)[N2], const c64 (&ediag)[NB]) {
+  auto build_row = [&](c64 (&m)[N2], const c64 (&ediag)[NB], const c64 z) {
 #pragma unroll
     for (int j = 0; j < NB; ++j) {
       const c64 dg = make_double2((j == a ? z.x : 0.0) - ediag[j].x, (j == a ? z.y : 0.0) - ediag[j].y);
@@ -121,6 +122,19 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
     }
   };
 
+  // Attempt 0 decimates at z itself.  Next to a pole of an isolated 2^k-cell segment the raw result can
+  // be off by ~1e-7, enough to push the spectral radius of the Newton operator P (.) Q past 1 for
+  // propagating modes (it is 1 - O(eta) at the fixed point), and then the doubling sum below diverges.
+  // Such a task (rare) is redone with the decimation at z + i*shift, which is well conditioned, and
+  // polished from there at the true z.  The whole CTA repeats; unaffected tasks recompute the same bits.
+  bool diverged = false;
+  double final_res = 0.0, final_scale = 1.0;
+  c64* Pb = Gt;                    // staging inside Gt once the inverse has been consumed
+  c64* Qb = Gt + MATN;
+  c64* Tb = Gt + 2 * MATN;
+  for (int attempt = 0; attempt < 2; ++attempt) {
+  const c64 zd = diverged ? make_double2(z.x, z.y + p.shift) : z;
+  bool div_now = false;
   c64 eh[NB];          // row a of eps_hh
   c64 es[NB];          // row a of eps_s,11 (half 1; half 0 keeps eps_s,00 = U I)
 #pragma unroll
@@ -137,7 +151,7 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
   for (int it = 0; it < p.maxit + 2; ++it) {
     {
       c64 m[N2];
-      build_row(m, eh);
+      build_row(m, eh, zd);
       const bool permuted = gj_invert<N2>(m, sm, t, r, live, p.theta2);
       store_inverse<N2>(m, Gt, sm, t, r, live, permuted);
     }
@@ -187,7 +201,7 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
     c64 m[N2], ed[NB];
 #pragma unroll
     for (int b = 0; b < NB; ++b) ed[b] = h == 0 ? make_double2(b == a ? U : 0.0, 0.0) : es[b];
-    build_row(m, ed);
+    build_row(m, ed, zd);
     const bool permuted = gj_invert<N2>(m, sm, t, r, live, p.theta2);
     store_inverse<N2>(m, Gt, sm, t, r, live, permuted);
 #pragma unroll
@@ -197,11 +211,8 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
   __syncthreads();
 
   // ---- Newton polish of X = g_surf,00 (header).  Gt holds a full inverse whose 00 block is X.
-  c64* Pb = Gt;                    // staging inside Gt once the inverse has been consumed
-  c64* Qb = Gt + MATN;
-  c64* Tb = Gt + 2 * MATN;
-  double final_res = 0.0, final_scale = 1.0;
-  for (int pass = 0; pass < kNewtonMax; ++pass) {
+  const int n_pass = attempt ? 2 * kNewtonMax : kNewtonMax;     // CTA-uniform
+  for (int pass = 0; pass < n_pass; ++pass) {
     c64 gold[NB];                  // row a of X (half 0)
     {
       c64 m[N2], ed[NB];
@@ -218,7 +229,7 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
         for (int b = 0; b < NB; ++b)
           if (b == a) ed[b].x += U;
       }
-      build_row(m, ed);
+      build_row(m, ed, z);
       const bool permuted = gj_invert<N2>(m, sm, t, r, live, p.theta2);
       store_inverse<N2>(m, Gt, sm, t, r, live, permuted);    // Gt = G(X)
     }
@@ -260,7 +271,7 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
     row_to<NB>((h == 0 ? Pb : Qb) + a * NB, pqrow, live);
     __syncthreads();
     bool pdone = false;
-    for (int it = 0; it < p.maxit + 2; ++it) {
+    for (int it = 0; it < kDoublingMax; ++it) {
       c64 w[NB];
       if (h == 0) {
         gemm_row<NB>(w, dlt, Qb);                            // D Q
@@ -299,6 +310,7 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
 #pragma unroll
       for (int i = 0; i < N2; ++i) tmax = fmax(tmax, sm.mag[t * N2 + i]);
       if (tmax < 1e-4) pdone = true;                         // |P_j| |Q_j| < 1e-8: series summed
+      if (!(tmax < 1e6)) { pdone = true; div_now = true; }   // growing powers: spectral radius > 1
       const bool all_done = __syncthreads_and(pdone || !live);
       if (h == 0) row_from<NB>(pqrow, Pb + a * NB);
       if (all_done) break;
@@ -307,9 +319,13 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
     __syncthreads();
     if (live0) {
 #pragma unroll
-      for (int b = 0; b < NB; ++b) Gt[a * N2 + b] = make_double2(gold[b].x + dlt[b].x, gold[b].y + dlt[b].y);
+      for (int b = 0; b < NB; ++b)
+        Gt[a * N2 + b] = div_now ? gold[b] : make_double2(gold[b].x + dlt[b].x, gold[b].y + dlt[b].y);
     }
     __syncthreads();
+  }
+  if (attempt == 1 || !__syncthreads_or(div_now && live)) break;
+  diverged = div_now;
   }
   if (active && r == 0 && !(final_res <= 1e-9 * final_scale)) atomicExch(p.noconv_flag, 1);
 
