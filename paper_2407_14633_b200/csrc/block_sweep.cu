@@ -329,11 +329,13 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
         fetch(P[u]);
         if (kq < NB) {
           const c64* brow = mat_t + kq * NB;
+          c64 bv[NB];
+#pragma unroll
+          for (int b = 0; b < NB; ++b) bv[b] = brow[b];
 #pragma unroll
           for (int b = 0; b < NB; ++b) {
-            const c64 bv = brow[b];
-            cfma(cc[0][b], av0, bv);
-            cfma(cc[1][b], av1, bv);
+            cfma(cc[0][b], av0, bv[b]);
+            cfma(cc[1][b], av1, bv[b]);
           }
         }
       }

@@ -194,3 +194,45 @@ def test_self_energy_kernel_vs_oracle():
                 err = np.abs(sig[c, :, lead] - ref).max(axis=(1, 2)) / scale
                 assert err.max() < 1e-12, (N, c, lead, err.max())
         h.negf_destroy()
+
+
+@pytest.mark.parametrize("cfg", [4, 5])
+def test_config4_and_5_full_length_sampled_vs_paper_recursion(cfg):
+    """configs[3] / configs[4] at their full device length (N = 2000 / 4000) and channel potentials, on
+    sampled channels and energies the oracle (tier O3) can do in seconds."""
+    wl = wlmod.make_config(cfg)
+    rng = np.random.default_rng(40 + cfg)
+    sub = wl.subset(neq_idx=np.sort(rng.choice(wl.K_neq, 5, replace=False)),
+                    eq_idx=np.sort(rng.choice(wl.K_eq, 3, replace=False)),
+                    channels=np.sort(rng.choice(wl.C, 2, replace=False)))
+    n_ref, T_ref = orgf.charge_and_transmission(sub, chunk=8)
+    n, T = _gpu_run(sub)
+    assert_parity(n, n_ref, f"config{cfg} sampled charge")
+    assert_parity(T, T_ref, f"config{cfg} sampled T(E)")
+
+
+def test_self_energy_next_to_a_segment_pole_regression():
+    """z - U_end = -0.33765527 + 1e-6 i sits ~1e-9 from a pole of an isolated 2^k-cell segment of the
+    decimation: the raw result is off by ~4e-7 and the Newton doubling sum used to diverge (NaN
+    self-energy in the config 4 loop).  The kernel must redo such a task and still match the oracle."""
+    import torch
+    from oracle import selfenergy as se
+    from paper_2407_14633_b200 import Negf
+    z0 = -0.3386878743069309 + 1e-6j
+    U0 = -0.001032601892690806
+    wl = wlmod.make_config(3, N=4, K_neq=3, K_eq=0)
+    wl.z_neq = np.array([z0, z0 + 1e-9, z0 - 1e-7])
+    wl.w_neq = np.ones(3)
+    wl.phi = np.array([[-U0, -U0, -U0 - 0.01, -U0 - 0.01]])
+    h = Negf.from_workload(wl)
+    h.negf_set_potential(torch.tensor(wl.phi, dtype=torch.float64, device="cuda"))
+    sig = torch.empty((1, 3, 2, wl.n * wl.n), dtype=torch.complex128, device="cuda")
+    h.negf_self_energy(sig)
+    h.negf_sync()
+    sig = sig.cpu().numpy().reshape(3, 2, wl.n, wl.n)
+    assert np.all(np.isfinite(sig.view(np.float64)))
+    sL, sR, _ = se.sigma_block(wl.z_neq, wl.coup_even, wl.coup_odd, wl.N, U0, U0 + 0.01)
+    for lead, ref in ((0, sL), (1, sR)):
+        err = np.abs(sig[:, lead] - ref).max() / np.abs(ref).max()
+        assert err < 1e-11, (lead, err)
+    h.negf_destroy()
