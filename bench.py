@@ -336,9 +336,9 @@ def run_ours(args):
         cpu_baseline = {"value": cpu_sps, "unit": UNIT, "cores": cores, "kind": "oracle",
                         "sample": desc + f" ({cpu_dt:.1f} s, oracle/negf_rgf.py)"}
 
-    # my kernels per step: negate + sweep batches + 2-level row reduce + mode reduce + Broyden
+    # my kernels per step: negf_set_potential + negf_charge (counted by the library's plan) + 4 Broyden
     plan = h.negf_get_plan()
-    my_launches = args.steps * (1 + plan["n_batches"] + 3 + 4)
+    my_launches = args.steps * (plan["kernel_launches"] + 4)
     value = units / (ms * 1e-3)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

@@ -144,7 +144,7 @@ typedef struct {
   int32_t n_batches;         /* launches of the sweep kernel per negf_charge             */
   int32_t sweeps_per_charge; /* C * chains * (K_eq + K_neq)                              */
   int32_t max_sr_iterations; /* largest Sancho-Rubio iteration count of the last set_potential (after sync) */
-  int32_t reserved;
+  int32_t kernel_launches;   /* kernels launched by one negf_set_potential + negf_charge pair               */
 } negf_plan_info;
 NEGF_API negf_status negf_get_plan(negf_handle* h, negf_plan_info* out);
 

@@ -61,7 +61,7 @@ class negf_kernel_stat(C.Structure):
 class negf_plan_info(C.Structure):
     _fields_ = [("history_bytes", C.c_int64), ("partial_bytes", C.c_int64),
                 ("n_batches", C.c_int32), ("sweeps_per_charge", C.c_int32),
-                ("max_sr_iterations", C.c_int32), ("reserved", C.c_int32)]
+                ("max_sr_iterations", C.c_int32), ("kernel_launches", C.c_int32)]
 
 
 _lib = None

@@ -327,6 +327,10 @@ void block_path_plan(BlockPath* bp, negf_plan_info* out) {
   out->partial_bytes = bp->partial_bytes;
   out->n_batches = bp->n_launches;
   out->max_sr_iterations = bp->last_max_iters;
+  // negate + Sancho-Rubio + sweep launches + one combine per launch that holds contour CTAs + 2-level reduce
+  int combines = 0;
+  for (long long begin = 0; begin < bp->n_eq_cta; begin += bp->slots) ++combines;
+  out->kernel_launches = 1 + 1 + bp->n_launches + combines + 2;
 }
 
 }  // namespace negf

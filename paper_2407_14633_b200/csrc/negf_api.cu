@@ -455,6 +455,16 @@ extern "C" negf_status negf_get_plan(negf_handle* h, negf_plan_info* out) {
     out->history_bytes = h->hist_bytes;
     out->partial_bytes = h->partial_bytes;
     out->n_batches = (int32_t)h->batches.size();
+    // negate + per batch (real-axis sweep [+ contour sweep + contour combine]) + 2-level row reduce + mode reduce
+    int launches = 1 + 3;
+    const int wpc = h->cwarps_per_channel + 2 * h->rwarps_per_channel;
+    for (const Batch& b : h->batches) {
+      bool has_c = false, has_r = false;
+      for (int w = b.warp_begin; w < b.warp_end && !(has_c && has_r); ++w)
+        ((w % wpc) < h->cwarps_per_channel ? has_c : has_r) = true;
+      launches += (has_r ? 1 : 0) + (has_c ? 2 : 0);
+    }
+    out->kernel_launches = launches;
   } else {
     block_path_plan(h->block, out);
   }
