@@ -83,6 +83,12 @@ struct SweepLaunch {
   CsrSet csr;
 };
 cudaError_t launch_block_sweep(int nb, const SweepLaunch& p, cudaStream_t s);
+// n = 17: the way back of the real-axis CTAs of a finished sweep launch on the FP64 tensor cores
+// (block_back.cu).  Other block sizes do the way back inside block_sweep_kernel.
+constexpr int kHistLd17 = 18;         // row stride of a history matrix: 288 B rows start on 32-byte sectors
+constexpr int kHistRec17 = 17 * kHistLd17;   // history elements per task and ring
+constexpr int kBackThreads17 = 224;   // 7 warps = the 7 tasks of one block_sweep CTA
+cudaError_t launch_block_back17(const SweepLaunch& p, cudaStream_t s);
 // Contour combine over the pairs of contour CTAs [cta_begin, cta_begin + 2 n_pairs) of a finished
 // sweep launch whose first CTA was launch_cta_begin.
 cudaError_t launch_block_combine(int nb, const SweepLaunch& p, long long pair_cta_begin, int n_pairs,

@@ -169,7 +169,32 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
   // entering step s is not diagonal, ytilde_{s-1} is also in the task's exchange matrix.
   c64 d[2][NB];
   c64* hp = hb;
-  for (int s = 0; s < N; ++s, hp += G::STEP_ELEMS) {
+  // n = 17, real-axis CTAs: ytilde_s goes out row-major (row stride 18: rows start on 32-byte sectors)
+  // with 32-byte stores, one full sector per lane and instruction; block_back.cu reads it back as
+  // DMMA fragments.  (16-byte stores at row-strided addresses cost 2.4x the L2 write sectors.)
+  c64* hrec = p.hist + (size_t)blockIdx.x * N * G::STEP_ELEMS + (size_t)t * kHistRec17;
+  auto store_row17 = [&](c64* dst, const c64 (&row)[NB]) {
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+      asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(dst + 2 * j), "d"(row[2 * j].x),
+                   "d"(row[2 * j].y), "d"(row[2 * j + 1].x), "d"(row[2 * j + 1].y)
+                   : "memory");
+    dst[16] = row[NB - 1];
+  };
+  auto store_history = [&](const c64 (&y)[2][NB]) {
+    if (!live) return;
+    if constexpr (NB == 17) {
+      store_row17(hrec + a * kHistLd17, y[0]);
+      if (valid1) store_row17(hrec + rid1 * kHistLd17, y[1]);
+    } else {
+#pragma unroll
+      for (int b = 0; b < NB; ++b) {
+        hp[(size_t)b * G::THREADS] = y[0][b];
+        if (valid1) hp[HQ + (size_t)b * G::THREADS] = y[1][b];
+      }
+    }
+  };
+  for (int s = 0; s < N; ++s, hp += G::STEP_ELEMS, hrec += G::STEP_ELEMS) {
     const int i = dir ? N - 1 - s : s;
     if (s == 0) {
 #pragma unroll
@@ -248,33 +273,25 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
           d[1][b] = cmul(d[1][b], kb);
         }
       }                                                            // last ring: G_(k,k) itself
-      if (!contour && live) {
-#pragma unroll
-        for (int b = 0; b < NB; ++b) {
-          hp[(size_t)b * G::THREADS] = d[0][b];
-          if (valid1) hp[HQ + (size_t)b * G::THREADS] = d[1][b];
-        }
-      }
+      if (!contour) store_history(d);
       __syncthreads();                                             // separates consecutive gj_invert2 calls
     } else {
       store_inverse2<NB>(d, mat_t, sm, t, a, live, permuted);
       __syncthreads();
       sparse_right_dagger2<NB>(d, Kpar[parn], mat_s, a, valid1);   // ytilde_s = g_s K_{s+1}^dagger
-      if (live) {
+      if (!contour) store_history(d);
+      if (live) {                                                  // only this thread reads its rows above
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
-          if (!contour) hp[(size_t)b * G::THREADS] = d[0][b];
           mat_t[a * NB + b] = d[0][b];
-          if (valid1) {
-            if (!contour) hp[HQ + (size_t)b * G::THREADS] = d[1][b];
-            mat_t[rid1 * NB + b] = d[1][b];
-          }
+          if (valid1) mat_t[rid1 * NB + b] = d[1][b];
         }
       }
       __syncthreads();
     }
   }
   if (contour) return;
+  if constexpr (NB == 17) return;   // the way back runs on the tensor cores: block_back.cu
 
   // ------------------------------------------------------------------ column recursion back
   const int R = p.geq + 2 * p.gneq;
@@ -539,6 +556,10 @@ static int ctas_per_sm_t(int nnz_cap) {
 }
 
 cudaError_t launch_block_sweep(int nb, const SweepLaunch& p, cudaStream_t s) {
+  if (nb == 17) {
+    cudaError_t e = launch_sweep_t<17>(p, s);
+    return e != cudaSuccess ? e : launch_block_back17(p, s);
+  }
   switch (nb) {
 #define NEGF_CASE(NB_) case NB_: return launch_sweep_t<NB_>(p, s);
     NEGF_BLOCK_SIZES(NEGF_CASE)
