@@ -115,18 +115,23 @@ __device__ __forceinline__ bool gj_invert(c64 (&r)[NB], const Smem<NB>& sm, int 
   bool used = false;
   bool any_search = false;
   c64 dinv = make_double2(1.0, 0.0);
-#pragma unroll
+  // The loop over elimination steps is not unrolled: after every step the registers are rotated by
+  // one column (folded into the destination registers of the elimination FMAs), so the pivot column
+  // is always register column 0 and the new inverse column enters at column NB-1; after NB steps the
+  // columns are back in order.  (Unrolled, the 2n = 34 wide inversions of sancho_rubio.cu are
+  // ~100 KB of code each and the kernel stalls on instruction fetch.)
+#pragma unroll 1
   for (int k = 0; k < NB; ++k) {
     const int buf = k & 1;
     c64* prow = sm.prow + ((size_t)buf * G::TPC + t) * (NB + 1);
     int bad = 0;
     if (a == k) {
-      const double m = cabs2(r[k]);
+      const double m = cabs2(r[0]);
       const bool accept = !used && (m >= thr) && (m > 0.0);
       if (accept) {
         const double rm = 1.0 / m;
-        dinv = make_double2(r[k].x * rm, -r[k].y * rm);
-        r[k] = make_double2(1.0, 0.0);
+        dinv = make_double2(r[0].x * rm, -r[0].y * rm);
+        r[0] = make_double2(1.0, 0.0);
         used = true;
         if (live) {
 #pragma unroll
@@ -144,20 +149,19 @@ __device__ __forceinline__ bool gj_invert(c64 (&r)[NB], const Smem<NB>& sm, int 
       // rare path: every task whose candidate was rejected searches column k over its unused rows
       any_search = true;
       const bool need = sm.ok[t] == 0;
-      if (need && live) sm.mag[t * NB + a] = used ? -1.0 : cabs2(r[k]);
+      if (need && live) sm.mag[t * NB + a] = used ? -1.0 : cabs2(r[0]);
       __syncthreads();
       if (need) {
         int best = 0;
         double bm = sm.mag[t * NB];
-#pragma unroll
         for (int i = 1; i < NB; ++i) {
           const double v = sm.mag[t * NB + i];
           if (v > bm) { bm = v; best = i; }
         }
         if (a == best) {
-          const double rm = 1.0 / cabs2(r[k]);
-          dinv = make_double2(r[k].x * rm, -r[k].y * rm);
-          r[k] = make_double2(1.0, 0.0);
+          const double rm = 1.0 / cabs2(r[0]);
+          dinv = make_double2(r[0].x * rm, -r[0].y * rm);
+          r[0] = make_double2(1.0, 0.0);
           used = true;
           if (live) {
 #pragma unroll
@@ -171,11 +175,17 @@ __device__ __forceinline__ bool gj_invert(c64 (&r)[NB], const Smem<NB>& sm, int 
       __syncthreads();
       p = sm.pk[buf * G::TPC + t];
     }
-    if (a != p) {
-      const c64 f = cmul(r[k], prow[NB]);
-      r[k] = make_double2(0.0, 0.0);
+    {
+      const bool piv = (a == p);
+      c64 f = cmul(r[0], prow[NB]);
+      if (piv) f = make_double2(0.0, 0.0);
 #pragma unroll
-      for (int j = 0; j < NB; ++j) cfms(r[j], f, prow[j]);
+      for (int j = 0; j + 1 < NB; ++j) {
+        c64 tmp = r[j + 1];
+        cfms(tmp, f, prow[j + 1]);
+        r[j] = tmp;
+      }
+      r[NB - 1] = make_double2((piv ? 1.0 : 0.0) - f.x, -f.y);
     }
   }
 #pragma unroll
