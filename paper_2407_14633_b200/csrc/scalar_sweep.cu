@@ -90,6 +90,11 @@ __device__ __forceinline__ void flush_tile(double (*tile)[33], int lane, int cnt
   __syncwarp();
 }
 
+// The way back met a step that the forward recursion rescaled (stored -h): undo the power of two.
+__device__ __noinline__ double cross_marker(double c2, double h) {
+  return c2 * ((fabs(h) >= 1.0) ? 0x1p-400 : 0x1p400);
+}
+
 __global__ void __launch_bounds__(kWarpsPerBlock * 32, 16)
 scalar_real_kernel(const ScalarLaunch p, const int n_warps) {
   __shared__ double tiles[kWarpsPerBlock][kTile][33];
@@ -226,31 +231,44 @@ scalar_real_kernel(const ScalarLaunch p, const int n_warps) {
     // |G_(i,k)|^2 = F_s h_s with F_{N-1} = 1/|D|^2, F_{s-1} = F_s * b2_s (* 2^-+400 across a marker).
     const int ring0 = dir ? 0 : N - 1;
     const int sign = dir ? 1 : -1;
-    for (int q0 = 0; q0 < N; q0 += kTile) {
-      const int cnt = min(kTile, N - q0);
+    // bond entering step ss = N-1-(q0+t): kTile is even, so its type depends on the parity of t only
+    const double b2_t_even = ((N - 1) & 1) ? b2_odd_s : b2_even_s;
+    const double b2_t_odd = ((N - 1) & 1) ? b2_even_s : b2_odd_s;
+    const double* __restrict__ hrd = hist + (size_t)(N - 1) * 32;   // walks down the history
+    double g2 = 0.0;
+    int q0 = 0;
+    for (; q0 + kTile <= N; q0 += kTile, hrd -= (size_t)kTile * 32) {   // full tiles: no tail tests
       double h[kTile];
 #pragma unroll
-      for (int t = 0; t < kTile; ++t) {
-        const int ss = N - 1 - (q0 + t);
-        h[t] = (t < cnt) ? hist[(size_t)ss * 32] : 0.0;
-      }
+      for (int t = 0; t < kTile; ++t) h[t] = *(hrd - (size_t)t * 32);
 #pragma unroll
       for (int t = 0; t < kTile; ++t) {
-        const int ss = N - 1 - (q0 + t);
-        const double hv = fabs(h[t]);
-        const double g2 = c2 * hv;                         // |G_(i,k)|^2
-        tile[t][lane] = (t < cnt) ? w_last * g2 : 0.0;
+        g2 = c2 * fabs(h[t]);                              // |G_(i,k)|^2
+        tile[t][lane] = w_last * g2;
+        if (__double2hiint(h[t]) < 0) c2 = cross_marker(c2, h[t]);   // rare: a rescaled step
+        c2 *= (t & 1) ? b2_t_odd : b2_t_even;
+      }
+      flush_tile(tile, lane, kTile, prow, ring0 + sign * q0, sign);
+    }
+    if (q0 < N) {                                          // ragged last tile
+      const int cnt = N - q0;
+#pragma unroll 1
+      for (int t = 0; t < kTile; ++t) {
+        double v = 0.0;
         if (t < cnt) {
-          if (ss == 0 && dir == 0 && active) {
-            // G_(0,N-1): transmission (eq.(5)), a4
-            p.T_part[((size_t)c * p.n_modes + mode) * p.K_neq + k] = __ldg(p.mode_w_T + mode) * gamL * gamR * g2;
-          }
-          if (h[t] < 0.0) c2 *= (hv >= 1.0) ? 0x1p-400 : 0x1p400;
-          c2 *= (ss & 1) ? b2_odd_s : b2_even_s;           // bond entering step ss
+          const double hv = *(hrd - (size_t)t * 32);
+          g2 = c2 * fabs(hv);
+          v = w_last * g2;
+          if (hv < 0.0) c2 = cross_marker(c2, hv);
+          c2 *= (t & 1) ? b2_t_odd : b2_t_even;
         }
+        tile[t][lane] = v;
       }
       flush_tile(tile, lane, cnt, prow, ring0 + sign * q0, sign);
     }
+    // the last value is |G_(first,last)|^2: transmission through the chain (eq.(5)), a4
+    if (dir == 0 && active)
+      p.T_part[((size_t)c * p.n_modes + mode) * p.K_neq + k] = __ldg(p.mode_w_T + mode) * gamL * gamR * g2;
   }
 }
 
