@@ -236,3 +236,17 @@ def test_self_energy_next_to_a_segment_pole_regression():
         err = np.abs(sig[:, lead] - ref).max() / np.abs(ref).max()
         assert err < 1e-11, (lead, err)
     h.negf_destroy()
+
+
+@pytest.mark.parametrize("N,K_neq,K_eq", [(2, 9, 3), (3, 8, 0), (5, 0, 6), (31, 15, 2)])
+def test_config3_degenerate_shapes(N, K_neq, K_eq):
+    """Shortest devices (N = 2, 3: both leads on adjacent rings; odd N flips the right lead's bond),
+    real-axis-only and contour-only handles, one more task than a CTA holds (15 = 2 x 7 + 1)."""
+    wl = wlmod.make_config(3, N=N, K_neq=max(K_neq, 1), K_eq=K_eq)
+    if K_neq == 0:
+        wl = wl.subset(neq_idx=[])
+    n_ref, T_ref = od.charge_and_transmission(wl)
+    n, T = _gpu_run(wl)
+    assert_parity(n, n_ref, "config3-degenerate charge")
+    if K_neq:
+        assert_parity(T, T_ref, "config3-degenerate T(E)")
