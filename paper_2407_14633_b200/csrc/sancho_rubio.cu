@@ -26,6 +26,8 @@
 //     dG00 = P dX Q,  P = G01 V1,  Q = V1^+ G10,   D - P D Q = G00 - X  summed by doubling
 //     (D += P D Q;  P <- P^2;  Q <- Q^2),
 // until the fixed-point residual is at rounding level (at most kNewtonMax passes).
+#include <math_constants.h>
+
 #include "block_ops.cuh"
 #include "block_path.h"
 #include "negf_internal.h"
@@ -61,10 +63,17 @@ __device__ __forceinline__ void row_to(c64* dst, const c64 (&r)[NB], bool pred) 
 }
 template <int NB>
 __device__ __forceinline__ double row_absmax(const c64 (&r)[NB]) {
+  // fmax drops NaNs, so a row with a NaN or an infinity reports +infinity explicitly: every
+  // convergence test downstream then fails instead of passing on garbage
   double m = 0.0;
+  bool finite = true;
 #pragma unroll
-  for (int b = 0; b < NB; ++b) m = fmax(m, fmax(fabs(r[b].x), fabs(r[b].y)));
-  return m;
+  for (int b = 0; b < NB; ++b) {
+    const double v = fmax(fabs(r[b].x), fabs(r[b].y));
+    finite = finite && (fabs(r[b].x) < CUDART_INF) && (fabs(r[b].y) < CUDART_INF);
+    m = fmax(m, v);
+  }
+  return finite ? m : CUDART_INF;
 }
 
 template <int NB>
@@ -182,7 +191,10 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
     for (int i = 0; i < N2; ++i) tmax = fmax(tmax, sm.mag[t * N2 + i]);
     if (!frozen) {
       ++iters;
-      if (remaining < 0) {
+      if (!(tmax < CUDART_INF)) {            // the decimation broke down (z on a pole of a segment)
+        div_now = true;
+        frozen = true;
+      } else if (remaining < 0) {
         if (tmax < p.tol) remaining = 2;
       } else {
         --remaining;
@@ -265,7 +277,7 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
     }
     final_res = tres;
     final_scale = tg;
-    const bool good = tres <= 2e-14 * tg;
+    const bool good = (tres <= 2e-14 * tg) && (tg < CUDART_INF) && !div_now;
     if (__syncthreads_and(good || !live)) break;            // Gt still holds G(X): X = its 00 block
     // stage P and Q inside Gt (the inverse is dead from here)
     row_to<NB>((h == 0 ? Pb : Qb) + a * NB, pqrow, live);

@@ -419,13 +419,18 @@ cudaError_t launch_scalar_sweep(const ScalarLaunch& p, cudaStream_t s) {
   };
   const int n_c = cw_before(p.warp_end) - cw_before(p.warp_begin);
   const int n_r = nwarps - n_c;
-  // The few contour warps are latency-bound (two dependent passes over N rings); they start first on
-  // the side stream and the real-axis kernel fills the rest of the machine beside them.
+  // The few contour warps are latency-bound (a dependent pass over N rings); they start first on the
+  // side stream, their combine kernel follows them there, and the real-axis kernel fills the rest of
+  // the machine beside both.
   cudaError_t e;
   if (n_c > 0) {
+    if (n_c & 1) return cudaErrorInvalidValue;             // batches never split a contour pair
     if ((e = cudaEventRecord(p.ev_fork, s)) != cudaSuccess) return e;
     if ((e = cudaStreamWaitEvent(p.side, p.ev_fork, 0)) != cudaSuccess) return e;
     scalar_contour_kernel<<<(n_c + kWarpsPerBlock - 1) / kWarpsPerBlock, kWarpsPerBlock * 32, 0, p.side>>>(p, n_c);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    dim3 grid((p.N + 127) / 128, n_c / 2);
+    scalar_combine_kernel<<<grid, 128, 0, p.side>>>(p, n_c / 2);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     if ((e = cudaEventRecord(p.ev_join, p.side)) != cudaSuccess) return e;
   }
@@ -433,13 +438,7 @@ cudaError_t launch_scalar_sweep(const ScalarLaunch& p, cudaStream_t s) {
     scalar_real_kernel<<<(n_r + kWarpsPerBlock - 1) / kWarpsPerBlock, kWarpsPerBlock * 32, 0, s>>>(p, n_r);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
   }
-  if (n_c > 0) {
-    if ((e = cudaStreamWaitEvent(s, p.ev_join, 0)) != cudaSuccess) return e;
-    if (n_c & 1) return cudaErrorInvalidValue;             // batches never split a contour pair
-    dim3 grid((p.N + 127) / 128, n_c / 2);
-    scalar_combine_kernel<<<grid, 128, 0, s>>>(p, n_c / 2);
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
-  }
+  if (n_c > 0 && (e = cudaStreamWaitEvent(s, p.ev_join, 0)) != cudaSuccess) return e;
   return cudaSuccess;
 }
 

@@ -220,18 +220,22 @@ def test_self_energy_next_to_a_segment_pole_regression():
     from paper_2407_14633_b200 import Negf
     z0 = -0.3386878743069309 + 1e-6j
     U0 = -0.001032601892690806
-    wl = wlmod.make_config(3, N=4, K_neq=3, K_eq=0)
-    wl.z_neq = np.array([z0, z0 + 1e-9, z0 - 1e-7])
-    wl.w_neq = np.ones(3)
-    wl.phi = np.array([[-U0, -U0, -U0 - 0.01, -U0 - 0.01]])
+    # second case (config 5 loop, right lead): the decimation itself breaks down to NaN, which fmax-based
+    # convergence tests used to swallow
+    z1 = 0.33736573920690816 + 1e-6j
+    U1 = -0.0002902289467536259
+    wl = wlmod.make_config(3, N=4, K_neq=4, K_eq=0)
+    wl.z_neq = np.array([z0, z0 + 1e-9, z0 - 1e-7, z1])
+    wl.w_neq = np.ones(4)
+    wl.phi = np.array([[-U0, -U0, -U1, -U1]])
     h = Negf.from_workload(wl)
     h.negf_set_potential(torch.tensor(wl.phi, dtype=torch.float64, device="cuda"))
-    sig = torch.empty((1, 3, 2, wl.n * wl.n), dtype=torch.complex128, device="cuda")
+    sig = torch.empty((1, 4, 2, wl.n * wl.n), dtype=torch.complex128, device="cuda")
     h.negf_self_energy(sig)
     h.negf_sync()
-    sig = sig.cpu().numpy().reshape(3, 2, wl.n, wl.n)
+    sig = sig.cpu().numpy().reshape(4, 2, wl.n, wl.n)
     assert np.all(np.isfinite(sig.view(np.float64)))
-    sL, sR, _ = se.sigma_block(wl.z_neq, wl.coup_even, wl.coup_odd, wl.N, U0, U0 + 0.01)
+    sL, sR, _ = se.sigma_block(wl.z_neq, wl.coup_even, wl.coup_odd, wl.N, U0, U1)
     for lead, ref in ((0, sL), (1, sR)):
         err = np.abs(sig[:, lead] - ref).max() / np.abs(ref).max()
         assert err < 1e-11, (lead, err)
