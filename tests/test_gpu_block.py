@@ -254,3 +254,32 @@ def test_config3_degenerate_shapes(N, K_neq, K_eq):
     assert_parity(n, n_ref, "config3-degenerate charge")
     if K_neq:
         assert_parity(T, T_ref, "config3-degenerate T(E)")
+
+
+def test_ideal_tube_integer_transmission_and_reciprocity_on_gpu():
+    """Pins P4 / P6 on the CUDA block path itself (no oracle involved): an ideal (17,0) tube has
+    T(E) = number of open subbands, |t| |1 - 2 cos(pi q/17)| < |E| < |t| |1 + 2 cos(pi q/17)|, to O(N eta);
+    (eta = 1e-6 as in every config)
+    and for real H the left-to-right and right-to-left columns give the same transmission, which here
+    shows as T being independent of which end the potential step sits on (mirror device)."""
+    import torch
+    from paper_2407_14633_b200 import Negf
+    E = np.array([0.2, 0.3, 0.6, 1.2, 3.0])
+    q = np.arange(17)
+    lo = 2.5 * np.abs(1.0 - 2.0 * np.abs(np.cos(np.pi * q / 17)))
+    hi = 2.5 * np.abs(1.0 + 2.0 * np.abs(np.cos(np.pi * q / 17)))
+    expected = np.array([np.sum((lo < e) & (e < hi)) for e in E], dtype=float)
+    wl = wlmod.make_config(3, N=24, K_neq=len(E), K_eq=0)
+    wl.z_neq = (E + 1e-6j).astype(np.complex128)
+    wl.w_neq = np.ones(len(E))
+    wl.phi[:] = 0.0
+    _, T = _gpu_run(wl)
+    assert np.allclose(T[0], expected, rtol=0, atol=1e-3), (T[0], expected)     # O(N eta / |t|) per mode
+    # mirror symmetry: a potential profile and its mirror image transmit equally (real symmetric H)
+    rng = np.random.default_rng(5)
+    wl.phi[0] = 0.2 * rng.normal(size=wl.N)
+    wl.z_neq = (E + 1e-6j).astype(np.complex128)
+    _, T1 = _gpu_run(wl)
+    wl.phi[0] = wl.phi[0][::-1].copy()
+    _, T2 = _gpu_run(wl)
+    assert_parity(T1, T2, "mirror device T(E)", rtol=1e-9)
