@@ -144,15 +144,15 @@ __device__ __forceinline__ void gj_phase2(c64 (&r)[2][NB], const Smem2<NB>& sm, 
       c64 f0 = cmul(r[0][0], inv), f1 = cmul(r[1][0], inv);
       if (piv0) f0 = make_double2(0.0, 0.0);
       if (piv1) f1 = make_double2(0.0, 0.0);
-      // all pivot-row loads are issued back to back (their latency is paid once), then the FMAs
-      c64 pr[NB];
-#pragma unroll
-      for (int j = 1; j < NB; ++j) pr[j] = prow[j];
+      // (hoisting or batching these loads in the source does not change the generated code: at 255
+      // registers the allocator keeps a single pivot-row element in flight, and each load's latency is
+      // exposed -- profiles/r01_final.md)
 #pragma unroll
       for (int j = 0; j + 1 < NB; ++j) {
+        const c64 pj = prow[j + 1];
         c64 t0 = r[0][j + 1], t1 = r[1][j + 1];
-        cfms(t0, f0, pr[j + 1]);
-        cfms(t1, f1, pr[j + 1]);
+        cfms(t0, f0, pj);
+        cfms(t1, f1, pj);
         r[0][j] = t0;
         r[1][j] = t1;
       }
