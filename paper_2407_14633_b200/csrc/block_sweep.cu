@@ -129,11 +129,11 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
   const int kk = contour ? k : p.K_eq + k;
   const c64 z = contour ? p.z_eq[k] : p.z_neq[k];
   const size_t K_all = (size_t)p.K_eq + p.K_neq;
-  const c64* tabL = p.table + (((size_t)id.c * K_all + kk) * 2 + 0) * 2 * G::MAT;
-  const c64* tabR = tabL + 2 * G::MAT;
-  const c64* tab_first = dir ? tabR : tabL;
-  const c64* tab_last = dir ? tabL : tabR;
-  const double* Uc = p.U + (size_t)id.c * N;
+  // Long-lived pointers are re-derived where they are used (ring 0, ring N-1, the history stores): the
+  // elimination loop needs every register it can get for the matrix rows and the pivot-row loads.
+  const size_t tab_off = (((size_t)id.c * K_all + kk) * 2 + 0) * 2 * G::MAT;
+#define NEGF_TAB_FIRST (p.table + tab_off + (dir ? 2 * G::MAT : 0))
+#define NEGF_TAB_LAST (p.table + tab_off + (dir ? 0 : 2 * G::MAT))
 
   // couplings of this direction, by parity of the bond: [0] even bond, [1] odd bond
   Csr Kgen[2];
@@ -168,11 +168,9 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
   // Loop invariant at the top of step s > 0: d = the thread's rows of ytilde_{s-1}; if the coupling
   // entering step s is not diagonal, ytilde_{s-1} is also in the task's exchange matrix.
   c64 d[2][NB];
-  c64* hp = hb;
   // n = 17, real-axis CTAs: ytilde_s goes out row-major (row stride 18: rows start on 32-byte sectors)
   // with 32-byte stores, one full sector per lane and instruction; block_back.cu reads it back as
   // DMMA fragments.  (16-byte stores at row-strided addresses cost 2.4x the L2 write sectors.)
-  c64* hrec = p.hist + (size_t)blockIdx.x * N * G::STEP_ELEMS + (size_t)t * kHistRec17;
   auto store_row17 = [&](c64* dst, const c64 (&row)[NB]) {
 #pragma unroll
     for (int j = 0; j < 8; ++j)
@@ -181,9 +179,11 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
                    : "memory");
     dst[16] = row[NB - 1];
   };
-  auto store_history = [&](const c64 (&y)[2][NB]) {
+  auto store_history = [&](const c64 (&y)[2][NB], int s) {
     if (!live) return;
+    c64* hp = hb + (size_t)s * G::STEP_ELEMS;
     if constexpr (NB == 17) {
+      c64* hrec = hp - tid + (size_t)t * kHistRec17;
       store_row17(hrec + a * kHistLd17, y[0]);
       if (valid1) store_row17(hrec + rid1 * kHistLd17, y[1]);
     } else {
@@ -194,12 +194,12 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
       }
     }
   };
-  for (int s = 0; s < N; ++s, hp += G::STEP_ELEMS, hrec += G::STEP_ELEMS) {
+  for (int s = 0; s < N; ++s) {
     const int i = dir ? N - 1 - s : s;
     if (s == 0) {
 #pragma unroll
       for (int b = 0; b < NB; ++b) {
-        const c64 s0 = tab_first[a * NB + b], s1 = tab_first[rid1 * NB + b];
+        const c64 s0 = NEGF_TAB_FIRST[a * NB + b], s1 = NEGF_TAB_FIRST[rid1 * NB + b];
         d[0][b] = make_double2(-s0.x, -s0.y);
         d[1][b] = valid1 ? make_double2(-s1.x, -s1.y) : make_double2(0.0, 0.0);
       }
@@ -217,6 +217,7 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
       }
       if (contour) {
         if (live) {
+          c64* hp = hb + (size_t)s * G::STEP_ELEMS;
 #pragma unroll
           for (int b = 0; b < NB; ++b) {
             hp[(size_t)b * G::THREADS] = d[0][b];
@@ -234,13 +235,13 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
     if (!contour && s == N - 1) {
 #pragma unroll
       for (int b = 0; b < NB; ++b) {
-        const c64 s0 = tab_last[a * NB + b], s1 = tab_last[rid1 * NB + b];
+        const c64 s0 = NEGF_TAB_LAST[a * NB + b], s1 = NEGF_TAB_LAST[rid1 * NB + b];
         d[0][b].x -= s0.x;
         d[0][b].y -= s0.y;
         if (valid1) { d[1][b].x -= s1.x; d[1][b].y -= s1.y; }
       }
     }
-    const double zu = z.x - Uc[i];
+    const double zu = z.x - p.U[(size_t)id.c * N + i];
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
       if (b == a) { d[0][b].x += zu; d[0][b].y += z.y; }
@@ -273,13 +274,13 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
           d[1][b] = cmul(d[1][b], kb);
         }
       }                                                            // last ring: G_(k,k) itself
-      if (!contour) store_history(d);
+      if (!contour) store_history(d, s);
       __syncthreads();                                             // separates consecutive gj_invert2 calls
     } else {
       store_inverse2<NB>(d, mat_t, sm, t, a, live, permuted);
       __syncthreads();
       sparse_right_dagger2<NB>(d, Kpar[parn], mat_s, a, valid1);   // ytilde_s = g_s K_{s+1}^dagger
-      if (!contour) store_history(d);
+      if (!contour) store_history(d, s);
       if (live) {                                                  // only this thread reads its rows above
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
@@ -299,7 +300,7 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
   const double f_last = fermi(z.x, dir ? p.mu_s : p.mu_d, p.kT);
   const double wt = active ? p.deg * p.w_neq[k] * (1.0 / (2.0 * kPi)) * f_last : 0.0;
   {
-    const c64* F_last = tab_last + G::MAT;
+    const c64* F_last = NEGF_TAB_LAST + G::MAT;
     if (live) {
 #pragma unroll
       for (int b = 0; b < NB; ++b) {
@@ -383,7 +384,7 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
   }
   // ------------------------------------------------------------------ transmission (direction 0)
   if (dir == 0) {
-    const c64* F_first = tab_first + G::MAT;
+    const c64* F_first = NEGF_TAB_FIRST + G::MAT;
     if (live) {
 #pragma unroll
       for (int b = 0; b < NB; ++b) {                               // C_0 = G_(0,N-1) F_R
