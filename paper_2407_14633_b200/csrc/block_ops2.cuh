@@ -70,7 +70,7 @@ struct Smem2 {
 // new inverse column enters at register column NB-1.  After all NB steps the columns are back in
 // their original order.  (A fully unrolled elimination is ~140 KB of code per inversion; with two
 // warps per scheduler the kernel then stalls on instruction fetch.)
-template <int NB, int Q>
+template <int NB>
 __device__ __forceinline__ void gj_phase2(c64 (&r)[2][NB], const Smem2<NB>& sm, int t, int a, bool live,
                                           const double (&thr)[2], bool (&used)[2], c64 (&dinv)[2], int kbeg,
                                           int kend, bool& any_search) {
@@ -82,24 +82,27 @@ __device__ __forceinline__ void gj_phase2(c64 (&r)[2][NB], const Smem2<NB>& sm, 
     const int buf = k & 1;
     c64* prow = sm.prow + ((size_t)buf * G::TPC + t) * G::PROW;
     int bad = 0;
-    if (a + Q * TPT == k) {
-      const double m = cabs2(r[Q][0]);
-      const bool accept = !used[Q] && (m >= thr[Q]) && (m > 0.0);
-      if (accept) {
-        const double rm = 1.0 / m;
-        dinv[Q] = make_double2(r[Q][0].x * rm, -r[Q][0].y * rm);
-        r[Q][0] = make_double2(1.0, 0.0);
-        used[Q] = true;
-        if (live) {
 #pragma unroll
-          for (int j = 0; j < NB; ++j) prow[j] = r[Q][j];
-          prow[NB] = dinv[Q];
-          sm.pk[buf * G::TPC + t] = k;
-          sm.perm[t * NB + k] = k;
+    for (int Q = 0; Q < 2; ++Q) {
+      if (a + Q * TPT == k) {
+        const double m = cabs2(r[Q][0]);
+        const bool accept = !used[Q] && (m >= thr[Q]) && (m > 0.0);
+        if (accept) {
+          const double rm = 1.0 / m;
+          dinv[Q] = make_double2(r[Q][0].x * rm, -r[Q][0].y * rm);
+          r[Q][0] = make_double2(1.0, 0.0);
+          used[Q] = true;
+          if (live) {
+#pragma unroll
+            for (int j = 0; j < NB; ++j) prow[j] = r[Q][j];
+            prow[NB] = dinv[Q];
+            sm.pk[buf * G::TPC + t] = k;
+            sm.perm[t * NB + k] = k;
+          }
         }
+        if (live) sm.ok[t] = accept ? 1 : 0;
+        bad = (live && !accept) ? 1 : 0;
       }
-      if (live) sm.ok[t] = accept ? 1 : 0;
-      bad = (live && !accept) ? 1 : 0;
     }
     int p = k;
     if (__syncthreads_or(bad)) {
@@ -188,8 +191,7 @@ __device__ __forceinline__ bool gj_invert2(c64 (&r)[2][NB], const Smem2<NB>& sm,
     dinv[q] = make_double2(1.0, 0.0);
   }
   bool any_search = false;
-  gj_phase2<NB, 0>(r, sm, t, a, live, thr, used, dinv, 0, TPT, any_search);
-  gj_phase2<NB, 1>(r, sm, t, a, live, thr, used, dinv, TPT, NB, any_search);
+  gj_phase2<NB>(r, sm, t, a, live, thr, used, dinv, 0, NB, any_search);
 #pragma unroll
   for (int q = 0; q < 2; ++q)
 #pragma unroll
