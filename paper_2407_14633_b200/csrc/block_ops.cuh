@@ -89,7 +89,7 @@ struct Smem {
 };
 
 // Default threshold of the diagonal-candidate test in gj_invert: the candidate pivot a_kk is accepted
-// when |a_kk|^2 >= theta2 * max_j |a_kj(0)|^2 (row k of the matrix as handed in); otherwise the task
+// when |a_kk|^2 >= theta2 * sum_j |a_kj(0)|^2 (row k of the matrix as handed in); otherwise the task
 // falls back to a full column search over its unused rows (partial pivoting).
 constexpr double kTheta2Default = 1e-6;
 
@@ -108,9 +108,9 @@ template <int NB>
 __device__ __forceinline__ bool gj_invert(c64 (&r)[NB], const Smem<NB>& sm, int t, int a, bool live,
                                           double theta2) {
   using G = Geo<NB>;
-  double thr = 0.0;
+  double thr = 0.0;                      // row scale: squared 2-norm (cheaper than a NaN-aware max)
 #pragma unroll
-  for (int j = 0; j < NB; ++j) thr = fmax(thr, cabs2(r[j]));
+  for (int j = 0; j < NB; ++j) thr = fma(r[j].x, r[j].x, fma(r[j].y, r[j].y, thr));
   thr *= theta2;
   bool used = false;
   bool any_search = false;

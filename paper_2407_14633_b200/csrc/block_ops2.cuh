@@ -169,7 +169,7 @@ __device__ __forceinline__ void gj_phase2(c64 (&r)[2][NB], const Smem2<NB>& sm, 
 // In-place Gauss-Jordan inversion, two rows per thread: r[q] is row a + q*TPT.  Same scheme as
 // gj_invert (block_ops.cuh): the pivot row is published raw with a 1 in the pivot column plus the
 // reciprocal pivot, every other row forms its own multiplier, all rows are scaled once at the end.
-// The diagonal candidate a_kk is accepted when |a_kk|^2 >= theta2 * max_j |a_kj(0)|^2, else the task
+// The diagonal candidate a_kk is accepted when |a_kk|^2 >= theta2 * sum_j |a_kj(0)|^2, else the task
 // searches column k over its unused rows.  On return thread a holds, in r[q], row perm^-1(a + q*TPT)
 // of the inverse with register column j being inverse column perm[j]; the return value says
 // (CTA-uniform) whether any task left the diagonal order (perm != identity possible).
@@ -184,9 +184,9 @@ __device__ __forceinline__ bool gj_invert2(c64 (&r)[2][NB], const Smem2<NB>& sm,
   c64 dinv[2];
 #pragma unroll
   for (int q = 0; q < 2; ++q) {
-    double m = 0.0;
+    double m = 0.0;                      // row scale: squared 2-norm (cheaper than a NaN-aware max)
 #pragma unroll
-    for (int j = 0; j < NB; ++j) m = fmax(m, cabs2(r[q][j]));
+    for (int j = 0; j < NB; ++j) m = fma(r[q][j].x, r[q][j].x, fma(r[q][j].y, r[q][j].y, m));
     thr[q] = m * theta2;
     dinv[q] = make_double2(1.0, 0.0);
   }

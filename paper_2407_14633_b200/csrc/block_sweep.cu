@@ -58,7 +58,7 @@ __device__ __forceinline__ CsrS csr_shared(const Csr& K) {
   return CsrS{smem_addr(K.rowptr), smem_addr(K.col), smem_addr(K.val)};
 }
 
-// y[q][b] = sum_{c in nz(K_rid)} K[rid][c] * X[c][b] for the thread's two rows (X in shared memory)
+// y[q][b] = - sum_{c in nz(K_rid)} K[rid][c] * X[c][b] for the thread's two rows (X in shared memory)
 template <int NB>
 __device__ __forceinline__ void sparse_left2(c64 (&y)[2][NB], const CsrS K, unsigned X, int a, bool valid1) {
   constexpr int TPT = Geo2<NB>::TPT;
@@ -74,7 +74,7 @@ __device__ __forceinline__ void sparse_left2(c64 (&y)[2][NB], const CsrS K, unsi
       const c64 v = lds_c64(K.val + 16 * e);
       const unsigned xr = X + (unsigned)lds_i32(K.col + 4 * e) * (NB * 16);
 #pragma unroll
-      for (int b = 0; b < NB; ++b) cfma(y[q][b], v, lds_c64(xr + 16 * b));
+      for (int b = 0; b < NB; ++b) cfms(y[q][b], v, lds_c64(xr + 16 * b));
     }
   }
 }
@@ -205,31 +205,28 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
       }
     } else {
       const int par = dir ? (i & 1) : ((i - 1) & 1);
+      // d := -K_s ytilde_{s-1} (the sign is folded into the product)
       if (kdiag[par]) {
         const c64 k0 = kd[par][a], k1 = kd[par][rid1];             // (K ytilde)_ab = K_aa ytilde_ab
+        const c64 n0 = make_double2(-k0.x, -k0.y), n1 = make_double2(-k1.x, -k1.y);
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
-          d[0][b] = cmul(k0, d[0][b]);
-          d[1][b] = cmul(k1, d[1][b]);
+          d[0][b] = cmul(n0, d[0][b]);
+          d[1][b] = cmul(n1, d[1][b]);
         }
       } else {
-        sparse_left2<NB>(d, Kpar[par], mat_s, a, valid1);          // K_s ytilde_{s-1}
+        sparse_left2<NB>(d, Kpar[par], mat_s, a, valid1);          // -K_s ytilde_{s-1}
       }
       if (contour) {
-        if (live) {
+        if (live) {                                                // the combine kernel reads +K ytilde
           c64* hp = hb + (size_t)s * G::STEP_ELEMS;
 #pragma unroll
           for (int b = 0; b < NB; ++b) {
-            hp[(size_t)b * G::THREADS] = d[0][b];
-            if (valid1) hp[HQ + (size_t)b * G::THREADS] = d[1][b];
+            hp[(size_t)b * G::THREADS] = make_double2(-d[0][b].x, -d[0][b].y);
+            if (valid1) hp[HQ + (size_t)b * G::THREADS] = make_double2(-d[1][b].x, -d[1][b].y);
           }
         }
         if (s == N - 1) break;
-      }
-#pragma unroll
-      for (int b = 0; b < NB; ++b) {
-        d[0][b] = make_double2(-d[0][b].x, -d[0][b].y);
-        d[1][b] = make_double2(-d[1][b].x, -d[1][b].y);
       }
     }
     if (!contour && s == N - 1) {
