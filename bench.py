@@ -54,7 +54,7 @@ def load_traffic(kernel: str, config: int):
 class ClockSampler(threading.Thread):
     """Samples SM clocks and throttle reasons with NVML during the timed region."""
 
-    def __init__(self, index: int, period: float = 0.05):
+    def __init__(self, index: int, period: float = 0.01):
         super().__init__(daemon=True)
         self.index, self.period = index, period
         self.samples, self.reasons = [], set()
@@ -368,12 +368,15 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=None,
+                    help="timed steps (default: 200 for the scalar configs, whose step is ~0.6 ms; 5 for config 3; 2 for configs 4-5)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config, 1-based")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-budget", type=float, default=15.0, dest="cpu_budget")
     args = ap.parse_args()
+    if args.steps is None:
+        args.steps = {1: 200, 2: 200, 3: 5}.get(args.config, 2) if args.impl == "ours" else 3
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3            # timing rule: W >= 3
     if args.impl == "reference":
