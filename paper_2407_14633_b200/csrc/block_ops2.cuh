@@ -63,8 +63,10 @@ struct Smem2 {
   }
 };
 
-// One phase of gj_invert2: elimination steps k = kbeg .. kend-1, whose diagonal pivot candidates all
-// live in row slot Q of thread a = k - Q*TPT.  The loop is NOT unrolled: after every step the thread's
+// The elimination steps k = kbeg .. kend-1 of gj_invert2; the diagonal pivot candidate of step k lives
+// in row slot Q = k / TPT of thread a = k - Q*TPT (both slots are tested at run time: ONE loop for all
+// steps -- compiled as one loop per slot the register allocator kept a single pivot-row load in
+// flight and exposed every load's latency).  The loop is NOT unrolled: after every step the thread's
 // registers are rotated by one column (the rotation is folded into the destination registers of the
 // elimination FMAs, it costs no instruction), so the pivot column is always register column 0 and the
 // new inverse column enters at register column NB-1.  After all NB steps the columns are back in
