@@ -283,3 +283,58 @@ def test_ideal_tube_integer_transmission_and_reciprocity_on_gpu():
     wl.phi[0] = wl.phi[0][::-1].copy()
     _, T2 = _gpu_run(wl)
     assert_parity(T1, T2, "mirror device T(E)", rtol=1e-9)
+
+
+def test_config3_full_launch_configuration():
+    """configs[2] at full size in the launch configuration bench.py times (2112 energies, 606 + 586
+    CTAs): T(E) of the full run against the oracle (tier O3) on sampled energies, and the charge
+    against properties that hold at any size -- it is linear in the energy set (full run = sum of
+    two runs on disjoint halves of the real-axis grid, the contour kept in the first), finite and
+    within the filling of the tube."""
+    wl = wlmod.config3()
+    n, T = _gpu_run(wl)
+    assert np.all(np.isfinite(n)) and np.all(np.isfinite(T))
+    assert np.all(n > 0.0) and np.all(n < 2.0 * wl.n)            # 0 .. deg * 17 electrons per ring
+    rng = np.random.default_rng(33)
+    ks = np.sort(rng.choice(wl.K_neq, 6, replace=False))
+    sub = wl.subset(neq_idx=ks, eq_idx=[])
+    _, T_ref = orgf.charge_and_transmission(sub, chunk=8)
+    assert_parity(T[:, ks], T_ref, "config3 full-run T(E) at sampled energies")
+    half = wl.K_neq // 2
+    n_a, _ = _gpu_run(wl.subset(neq_idx=np.arange(half)))
+    n_b, _ = _gpu_run(wl.subset(neq_idx=np.arange(half, wl.K_neq), eq_idx=[]))
+    assert_parity(n, n_a + n_b, "config3 full-run charge vs sum over energy halves", rtol=1e-12)
+
+
+def test_config4_full_launch_configuration():
+    """configs[3] at full size (16 channels x 2000 rings x 4160 energies, 17 sweep launches): sampled
+    T(E) against the oracle, linearity of the charge in the energy set, bounds."""
+    wl = wlmod.config4()
+    n, T = _gpu_run(wl)
+    assert np.all(np.isfinite(n)) and np.all(np.isfinite(T))
+    assert np.all(n > 0.0) and np.all(n < 2.0 * wl.n)
+    rng = np.random.default_rng(44)
+    ks = np.sort(rng.choice(wl.K_neq, 4, replace=False))
+    cs = np.sort(rng.choice(wl.C, 2, replace=False))
+    sub = wl.subset(neq_idx=ks, eq_idx=[], channels=cs)
+    _, T_ref = orgf.charge_and_transmission(sub, chunk=8)
+    assert_parity(T[np.ix_(cs, ks)], T_ref, "config4 full-run T(E) at sampled channels / energies")
+    half = wl.K_neq // 2
+    n_a, _ = _gpu_run(wl.subset(neq_idx=np.arange(half)))
+    n_b, _ = _gpu_run(wl.subset(neq_idx=np.arange(half, wl.K_neq), eq_idx=[]))
+    assert_parity(n, n_a + n_b, "config4 full-run charge vs sum over energy halves", rtol=1e-12)
+
+
+def test_config5_full_launch_configuration():
+    """configs[4] at full size (64 channels x 4000 rings x 8320 energies, one negf_charge of the loop):
+    sampled T(E) against the oracle, bounds."""
+    wl = wlmod.config5()
+    n, T = _gpu_run(wl)
+    assert np.all(np.isfinite(n)) and np.all(np.isfinite(T))
+    assert np.all(n > 0.0) and np.all(n < 2.0 * wl.n)
+    rng = np.random.default_rng(55)
+    ks = np.sort(rng.choice(wl.K_neq, 3, replace=False))
+    cs = np.sort(rng.choice(wl.C, 2, replace=False))
+    sub = wl.subset(neq_idx=ks, eq_idx=[], channels=cs)
+    _, T_ref = orgf.charge_and_transmission(sub, chunk=8)
+    assert_parity(T[np.ix_(cs, ks)], T_ref, "config5 full-run T(E) at sampled channels / energies")
