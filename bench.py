@@ -269,14 +269,31 @@ def run_ours(args):
     sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
-    e0.record(stream)
-    for _ in range(args.steps):
-        step()
-    e1.record(stream)
-    torch.cuda.synchronize()
+    # Timing rule: inputs larger than L2, or flush it.  The recursion history written and re-read by
+    # every step is >> 126 MB for configs 2-5; config 1 (1.6 MB) gets an explicit flush between steps,
+    # timed per step so that the flush stays outside the events.
+    small = h.negf_get_plan()["history_bytes"] < 2 * 126 * 2 ** 20
+    if small:
+        flush = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device=dev)
+        local_ms = 0.0
+        for _ in range(args.steps):
+            flush.zero_()
+            e0.record(stream)
+            step()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            local_ms += e0.elapsed_time(e1)
+        l2_note = "L2 flushed between steps (256 MB memset outside the per-step CUDA events)"
+    else:
+        e0.record(stream)
+        for _ in range(args.steps):
+            step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        local_ms = e0.elapsed_time(e1)
+        l2_note = None
     dist_barrier(world)
     clocks = sampler.stop()
-    local_ms = e0.elapsed_time(e1)
     stats = h.negf_kernel_stats(reset=True)
     n_final = n.cpu().numpy()
     assert np.all(np.isfinite(n_final)), "non-finite charge in the timed loop"
@@ -347,7 +364,7 @@ def run_ours(args):
         "config": {"workload": f"configs[{args.config - 1}] {wl.name}", "C": wl.C, "N": wl.N,
                    "block": wl.n, "n_modes": wl.n_modes, "K_neq": wl.K_neq, "K_eq": wl.K_eq,
                    "sweeps_per_step": sweeps_per_step, "parallelism": f"replicas x{world}",
-                   "l2": "recursion history %.2f GB per step >> 126 MB L2 (no flush needed)" % (
+                   "l2": l2_note or "recursion history %.2f GB per step >> 126 MB L2 (no flush needed)" % (
                        plan["history_bytes"] / 1e9),
                    "step": "set_potential+charge+transmission+poisson_stand_in+broyden_step"},
         "clocks": clocks,
