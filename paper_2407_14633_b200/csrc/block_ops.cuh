@@ -1,11 +1,11 @@
-// Device primitives of the block (n x n, real-space) path: thread geometry, shared-memory layout,
-// in-register Gauss-Jordan inversion, sparse coupling products and block reductions.
+// Device primitives shared by the block (n x n, real-space) kernels: complex helpers, the one-row-per-
+// thread geometry and Gauss-Jordan inversion used by sancho_rubio.cu (2n x 2n matrices), CSR tables
+// in shared memory, block reductions.  The sweep kernels use the two-rows-per-thread geometry of
+// block_ops2.cuh.
 //
-// Geometry: one thread owns one ROW of its task's n x n complex matrix
-// in registers; n consecutive threads form a task (one (channel, energy, direction) recursion);
-// TPC tasks share a CTA and advance ring by ring in lock step.  Tasks straddle warp boundaries
-// (17 does not divide 32), so rows are exchanged through shared memory and CTA barriers, never
-// through shuffles.  With n = 17: 15 tasks = 255 live threads + 1 ghost thread per 256-thread CTA.
+// One-row geometry: one thread owns one ROW of its task's matrix in registers; NB consecutive threads
+// form a task; TPC tasks share a CTA and advance in lock step.  Tasks straddle warp boundaries, so
+// rows are exchanged through shared memory and CTA barriers, never through shuffles.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -210,33 +210,6 @@ __device__ __forceinline__ void store_inverse(const c64 (&r)[NB], c64* mat_t, co
       if (perm[k] == a) row = k;
 #pragma unroll
     for (int j = 0; j < NB; ++j) mat_t[row * NB + perm[j]] = r[j];
-  }
-}
-
-// y[b] = sum_{c in nz(K_a)} K[a][c] * X[c][b]      (row a of K X, X in shared memory)
-template <int NB>
-__device__ __forceinline__ void sparse_left(c64 (&y)[NB], const Csr& K, const c64* X, int a) {
-#pragma unroll
-  for (int b = 0; b < NB; ++b) y[b] = make_double2(0.0, 0.0);
-  const int e1 = K.rowptr[a + 1];
-  for (int e = K.rowptr[a]; e < e1; ++e) {
-    const c64 v = K.val[e];
-    const c64* xr = X + K.col[e] * NB;
-#pragma unroll
-    for (int b = 0; b < NB; ++b) cfma(y[b], v, xr[b]);
-  }
-}
-
-// y[b] = sum_{d in nz(K_b)} xrow[d] * conj(K[b][d])   (row of X K^dagger, xrow = this thread's row in
-// shared memory)
-template <int NB>
-__device__ __forceinline__ void sparse_right_dagger(c64 (&y)[NB], const Csr& K, const c64* xrow) {
-#pragma unroll
-  for (int b = 0; b < NB; ++b) {
-    c64 acc = make_double2(0.0, 0.0);
-    const int e1 = K.rowptr[b + 1];
-    for (int e = K.rowptr[b]; e < e1; ++e) cfma(acc, xrow[K.col[e]], cconj(K.val[e]));
-    y[b] = acc;
   }
 }
 

@@ -29,9 +29,6 @@ struct Geo2 {
   // real-axis CTAs store, in the same space, TPC row-major matrices of kHistRec17 elements (block_back.cu)
   static constexpr long long STEP_ELEMS = 2LL * NB * THREADS;
   static_assert(NB != 17 || TPC * 306 <= 2 * NB * THREADS, "row-major records must fit the step");
-  // chunks of the history row that the way back streams through registers (even count)
-  static constexpr int NCH = 2 * ((NB + 5) / 6);
-  static constexpr int CH = (NB + NCH - 1) / NCH;
 };
 
 template <int NB>

@@ -415,6 +415,9 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
   }
 }
 
+#undef NEGF_TAB_FIRST
+#undef NEGF_TAB_LAST
+
 // Contour combine: G_(i,i) = [alpha_i - x_i - y_i]^-1 (Alg.1 step 1) and the first term
 // of eq.(4): -(deg/pi) Im[W_k Tr G_(i,i)].  grid = (ring chunks, pairs of contour sweep CTAs).
 template <int NB>
