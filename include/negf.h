@@ -166,9 +166,10 @@ NEGF_API negf_status broyden_destroy(broyden_handle* h);
 NEGF_API negf_status negf_fp64_peak(double* dfma_tflops, double* dmma_tflops);
 
 /* Diagnostic / test hook of the block path's in-register Gauss-Jordan inversion: a diagonal pivot
- * candidate is accepted when |a_kk| >= theta * max_j |a_kj|, otherwise the task searches the whole
- * column (partial pivoting).  theta <= 0 restores the default (1e-3); a huge theta (e.g. 1e150) forces
- * the search at every elimination step.  Process-wide; affects kernels launched afterwards. */
+ * candidate is accepted when |a_kk| >= theta * ||row k of the matrix handed in||_2, otherwise the task
+ * searches the whole column (partial pivoting).  theta <= 0 restores the default (1e-3); a huge theta
+ * (e.g. 1e150) forces the search at every elimination step.  Process-wide; affects kernels launched
+ * afterwards. */
 NEGF_API negf_status negf_set_pivot_threshold(double theta);
 
 /* Last error text of the calling thread (static storage, never NULL). */
