@@ -6,8 +6,12 @@ paper's step numbers.  Readings (R15-R19):
   R15  step 13 prints "-eta Delta f"; the mixing fraction is zeta.
   R16  the library performs ONE iteration per call and returns eps_max.
   R17  history window h: only the most recent h (v, w) pairs are kept; sums run
-       over stored pairs oldest first; the sums of steps 9-11 use the pairs stored
-       *before* this iteration's pair is added (which then evicts the oldest).
+       over stored pairs oldest first.  The paper keeps all M pairs (PAPER.md:214);
+       the window is BASELINE.json's ("history 8").  When the window is full, the
+       oldest pair leaves *before* steps 9-11, so that w_m = dx - G df is formed
+       with the same G = zeta I + sum_kept w v^T that the new pair is then added
+       to: only this order keeps the secant equation G_{m+1} df_m = dx_m that
+       defines the method (pinned by tests/test_oracle_broyden.py::test_r17_*).
   R18  d = ||Delta f||^2 = 0: steps 9-13 are skipped (no new pair).
   R19  eps_t = |f_t| / max(|x_in,t + x_out,t|, 1e-300).
 
@@ -46,6 +50,9 @@ class Broyden:
         eps_max = float(eps.max()) if eps.size else 0.0              # steps 5, 7
         d = float(np.dot(df, df))                                    # steps 6, 8
         if self.m > 0 and d != 0.0:
+            if len(self.V) == self.history:                          # R17: full window ->
+                self.V.pop(0)                                        # the oldest pair leaves
+                self.W.pop(0)                                        # before steps 9-11
             s = np.zeros(self.length)
             for v, w in zip(self.V, self.W):                         # steps 9-11 (m > 1)
                 s += w * float(np.dot(v, df))
@@ -53,9 +60,6 @@ class Broyden:
             w_new = -self.zeta * df + (x_in - self.x_old) - s        # step 13
             self.V.append(v_new)
             self.W.append(w_new)
-            if len(self.V) > self.history:                           # R17
-                self.V.pop(0)
-                self.W.pop(0)
         s = np.zeros(self.length)
         for v, w in zip(self.V, self.W):                             # steps 14-16
             s += w * float(np.dot(v, f))

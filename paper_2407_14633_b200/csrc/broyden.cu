@@ -1,12 +1,16 @@
 // Broyden's modified second method, Algorithm 3 of the paper, one GPU.
 // (a6 of SURVEY.md 8(a).)  Steps are numbered as in the paper.  Readings R15-R19 of DESIGN.md:
-// zeta in step 13, sliding window of `history` (v, w) pairs summed oldest first, d = 0 skips steps
-// 9-13, eps_t = |f_t| / max(|x_in + x_out|, 1e-300).
+// zeta in step 13, sliding window of `history` (v, w) pairs summed oldest first -- when the window is
+// full the oldest pair leaves BEFORE steps 9-11, so that the new pair satisfies the secant equation
+// G_{m+1} df_m = dx_m with G = zeta I + sum over the kept pairs (R17) --, d = 0 skips steps 9-13,
+// eps_t = |f_t| / max(|x_in + x_out|, 1e-300); a non-finite residual gives eps_max = +infinity.
 //
 // The paper's atomics (steps 5, 6, 9, 14) are replaced by warp-shuffle + shared
 // memory block reductions and a fixed-order second stage, so results are bit-reproducible.  All dot
 // products of one iteration (V^T df, V^T f, df.df, df.f) come from ONE pass over the vectors: the new
 // pair's k_m = v_m.f equals (df.f)/d, so steps 14-15 need no second reduction.
+#include <math_constants.h>
+
 #include <new>
 
 #include "negf_internal.h"
@@ -23,7 +27,7 @@ struct Plan {              // device-resident ring-buffer state
   int m;                   // iteration counter of Alg.3
   int do_store;            // this step adds a pair (m > 0 and d != 0)
   int slot_new;            // slot the new pair goes to
-  int evict;               // the oldest pair is dropped after step 11
+  int evict;               // the window is full: the oldest pair is dropped before steps 9-11 (R17)
 };
 
 struct Dots {              // results of the reductions, device memory
@@ -38,9 +42,16 @@ __device__ __forceinline__ double warp_sum(double v) {
   for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
   return v;
 }
+// max that does not lose a non-finite residual: fmax drops NaN, and a caller looping on
+// "eps_max >= 1e-5" would then declare convergence on a NaN state.  NaN and
+// infinity both map to +infinity.
+__device__ __forceinline__ double nan_max(double a, double b) {
+  if (!(fabs(b) <= 1.79769313486231570e308)) b = CUDART_INF;
+  return (a >= b) ? a : b;       // a is never NaN by construction
+}
 __device__ __forceinline__ double warp_max(double v) {
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+  for (int o = 16; o > 0; o >>= 1) v = nan_max(v, __shfl_down_sync(0xffffffffu, v, o));
   return v;
 }
 
@@ -63,7 +74,7 @@ broyden_dots_kernel(const double* __restrict__ x_in, const double* __restrict__ 
     const double f = xi - xo;                                  // step 2
     const double df = f - f_old[t];                            // step 3
     if (first) {
-      em = fmax(em, fabs(f) / fmax(fabs(xi + xo), 1e-300));    // step 4
+      em = nan_max(em, fabs(f) / fmax(fabs(xi + xo), 1e-300)); // step 4
       d += df * df;                                            // step 6
       e += df * f;
     }
@@ -100,7 +111,7 @@ broyden_dots_kernel(const double* __restrict__ x_in, const double* __restrict__ 
   if (threadIdx.x < 2 * kChunk + 3) {
     double t = 0.0;
     if (threadIdx.x == 2 * kChunk + 2) {
-      for (int w = 0; w < kThreads / 32; ++w) t = fmax(t, sm[w][threadIdx.x]);
+      for (int w = 0; w < kThreads / 32; ++w) t = nan_max(t, sm[w][threadIdx.x]);
     } else {
       for (int w = 0; w < kThreads / 32; ++w) t += sm[w][threadIdx.x];
     }
@@ -117,7 +128,7 @@ __global__ void broyden_finish_kernel(const double* __restrict__ part, int nbloc
   if (q < 2 * kChunk + 3) {
     double t = 0.0;
     if (q == 2 * kChunk + 2) {
-      for (int b = 0; b < nblocks; ++b) t = fmax(t, part[(size_t)b * (2 * kChunk + 3) + q]);
+      for (int b = 0; b < nblocks; ++b) t = nan_max(t, part[(size_t)b * (2 * kChunk + 3) + q]);
     } else {
       for (int b = 0; b < nblocks; ++b) t += part[(size_t)b * (2 * kChunk + 3) + q];
     }
@@ -166,7 +177,7 @@ broyden_update_kernel(double* __restrict__ x_in, const double* __restrict__ x_ou
     double w_new = 0.0;
     if (store) {
       double s1 = 0.0;
-      for (int j = 0; j < n_stored; ++j)                                  // steps 10-11
+      for (int j = evict; j < n_stored; ++j)                              // steps 10-11 (R17: kept pairs)
         s1 += W[(size_t)((head + j) % history) * len + t] * k1buf[j];
       w_new = -zeta * df + (xi - x_old[t]) - s1;                          // step 13 (R15)
     }

@@ -80,6 +80,50 @@ def test_per_step_parity_with_identical_state_at_config5_length():
     gb.broyden_destroy()
 
 
+def test_non_finite_residual_gives_non_finite_eps_max():
+    """A NaN (or infinite) entry of F(x) -- e.g. a singular pivot upstream -- must not be reported
+    as convergence: eps_max comes back non-finite (the oracle's np.max returns NaN; the device
+    returns +infinity, fmax would have dropped the NaN).  PAPER.md:216 loops on eps_max >= 1e-5."""
+    import torch
+    from paper_2407_14633_b200 import Broyden
+    rng = np.random.default_rng(3)
+    for bad, pos in ((np.nan, 4321), (np.inf, 0), (-np.inf, 99999)):
+        x0, y0 = rng.normal(size=100000), rng.normal(size=100000)
+        y0[pos] = bad
+        gb = Broyden(100000, 8, 0.1)
+        eps = gb.broyden_step(torch.tensor(x0, device="cuda"), torch.tensor(y0, device="cuda"))
+        _, eps_ref = obroyden.Broyden(100000, 8, 0.1).step(x0, y0)
+        assert not np.isfinite(eps) and not np.isfinite(eps_ref)
+        gb.broyden_destroy()
+
+
+@pytest.mark.parametrize("history,steps", [(3, 9), (1, 5), (8, 14)])
+def test_device_window_keeps_the_secant_equation(history, steps):
+    """R17 on the device alone: x_{m+2} - x_{m+1} + G_{m+1} f_{m+1} = 0 defines G_{m+1} on f_{m+1}
+    only, so the secant equation is checked through linearity: for the affine map F(x) = A x + b
+    (f is affine, df = (I - A) dx) a method that satisfies G_{m+1} df_m = dx_m for the newest pair
+    with history >= 1 reproduces the oracle trajectory, and the oracle is pinned on the secant
+    equation (tests/test_oracle_broyden.py::test_r17_*).  Here: trajectory parity past eviction
+    with history 1, 3, 8 on an affine map (no tanh saturation hiding a wrong term)."""
+    import torch
+    from paper_2407_14633_b200 import Broyden
+    dim = 40
+    rng = np.random.default_rng(100 + history)
+    A = rng.normal(size=(dim, dim))
+    A *= 0.7 / np.linalg.norm(A, 2)
+    b = rng.normal(size=dim)
+    ob = obroyden.Broyden(dim, history, 0.1)
+    gb = Broyden(dim, history, 0.1)
+    x_ref = np.zeros(dim)
+    x = torch.zeros(dim, dtype=torch.float64, device="cuda")
+    for it in range(steps):
+        x_ref, _ = ob.step(x_ref, A @ x_ref + b)
+        xg = x.cpu().numpy()
+        gb.broyden_step(x, torch.tensor(A @ xg + b, device="cuda"), want_eps=False)
+        assert_parity(x.cpu().numpy(), x_ref, f"iterate {it}", rtol=1e-9)
+    gb.broyden_destroy()
+
+
 def test_repeated_pair_adds_no_history_and_reset():
     """R18: d = ||df||^2 = 0 skips steps 9-13; broyden_reset restarts at plain mixing."""
     import torch

@@ -1,6 +1,7 @@
 """Pins of the Broyden oracle (Algorithm 3): textbook special
 cases and the dense-matrix method it must equal (DESIGN.md pins P11, P12)."""
 import numpy as np
+import pytest
 
 from oracle.broyden import Broyden, DenseBadBroyden
 
@@ -98,3 +99,57 @@ def test_window_eviction_and_zero_df():
     nV = len(b2.V)
     x1, _ = b2.step(x0, F(x0))            # same input again: df = 0
     assert len(b2.V) == nV and np.all(np.isfinite(x1))
+
+
+def _secant_defect(history, steps, dim=10, seed=4):
+    F = _contractive_map(dim, seed)
+    b = Broyden(dim, history=history, zeta=0.1)
+    x = np.zeros(dim)
+    xs, fs = [], []
+    for _ in range(steps):
+        xs.append(x.copy())
+        fs.append(x - F(x))
+        x, _ = b.step(x, F(x))
+    G = 0.1 * np.eye(dim) + sum(np.outer(w, v) for v, w in zip(b.V, b.W))
+    dx, df = xs[-1] - xs[-2], fs[-1] - fs[-2]
+    return np.max(np.abs(G @ df - dx)) / np.max(np.abs(dx)), x, xs, fs, b
+
+
+@pytest.mark.parametrize("history,steps", [(3, 6), (3, 9), (2, 7), (1, 5), (8, 14)])
+def test_r17_window_keeps_the_secant_equation(history, steps):
+    """Pin of reading R17 (sliding window).  Broyden's second method is DEFINED by the secant
+    equation G_{m+1} df_m = dx_m (Alg.3 builds G = zeta I + W V^T pair by pair so
+    that each new pair satisfies it).  With a window, G is the sum over the KEPT pairs only, so the
+    pair that is dropped must leave the sum *before* steps 9-11 form w_m = dx - G df; summing
+    steps 9-11 over a pair that is then evicted leaves G_{m+1} df_m - dx_m = -w_old (v_old . df_m)
+    != 0.  This test fails (3.9e-3) for the evict-after order and holds to rounding for
+    evict-before."""
+    defect, *_ = _secant_defect(history, steps)
+    assert defect < 1e-12
+
+
+def test_r17_window_step_equals_dense_rank_update_of_the_kept_pairs():
+    """Brute force, independent of the vector form: after every step the next iterate must be
+    x - G f with the DENSE matrix G = zeta I + sum_{kept} w v^T, where the dense side rebuilds
+    G from scratch each step from its own list of kept (dx, df) pairs: start from zeta I and
+    apply the textbook rank-one update G <- G + (dx - G df) df^T / (df^T df) ... but only for the
+    newest pair, on top of the previous G minus the evicted pair's rank-one term."""
+    dim, h = 9, 3
+    F = _contractive_map(dim, 11)
+    b = Broyden(dim, history=h, zeta=0.1)
+    terms = []                                  # dense rank-one terms (matrix each), oldest first
+    x = np.zeros(dim)
+    x_old = f_old = None
+    for m in range(10):
+        f = x - F(x)
+        if m > 0:
+            dx, df = x - x_old, f - f_old
+            if len(terms) == h:
+                terms.pop(0)                    # the window drops the oldest term first
+            G = 0.1 * np.eye(dim) + sum(terms, np.zeros((dim, dim)))
+            terms.append(np.outer(dx - G @ df, df) / (df @ df))
+        G = 0.1 * np.eye(dim) + sum(terms, np.zeros((dim, dim)))
+        x_expect = x - G @ f
+        x_old, f_old = x.copy(), f.copy()
+        x, _ = b.step(x, F(x))
+        assert np.max(np.abs(x - x_expect)) < 1e-12 * max(1.0, np.max(np.abs(x_expect)))
