@@ -159,6 +159,50 @@ def test_p2_surface_gf_is_fixed_point_of_adding_a_layer():
         assert np.all(np.linalg.eigvalsh((g[k] - g[k].conj().T) / 2j) < 1e-9)   # retarded: Im g <= 0
 
 
+@pytest.mark.parametrize("N,n,seed", [(4, 3, 0), (5, 3, 1), (5, 2, 2), (3, 4, 3)])
+def test_p2_block_leads_brute_force_non_commuting_couplings(N, n, seed):
+    """Brute force of the block-lead construction (eq.(2), PAPER.md:79: Sigma = tau^dagger g tau;
+    decimation; readings R7, R9).  On the (17,0) tube every coupling commutes, so a
+    dagger/transpose or left/right mix-up in ``block_lead_layers`` / ``sigma_block`` would be
+    invisible there.  Here the couplings are random complex NON-commuting n x n blocks; the leads are
+    written out explicitly as L rings per side continuing the even/odd bond pattern of the device
+    (bond (j, j+1) is coup_even for even j, coup_odd for odd j, for every integer j) at the end
+    ring's on-site energy, and the whole (N + 2L) n matrix is inverted densely.  Its device block
+    must equal the Green's function the oracle gets from Sancho-Rubio self-energies.  eta = 0.4
+    makes the truncation error exp(-O(L eta)) negligible at L = 320."""
+    rng = np.random.default_rng(300 + seed)
+    ce = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    co = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    assert np.max(np.abs(ce @ co - co @ ce)) > 0.1          # the point of the test
+    U = rng.uniform(-0.5, 0.5, N)
+    L = 320
+    tot = N + 2 * L
+
+    def bond(j):                                              # H_{j,j+1}, j any integer
+        return ce if j % 2 == 0 else co
+
+    for z in (0.37 + 0.4j, -1.1 + 0.4j):
+        Hbig = np.zeros((tot * n, tot * n), dtype=np.complex128)
+        for r in range(tot):
+            j = r - L                                         # ring index; device is 0 .. N-1
+            Uj = U[0] if j < 0 else (U[N - 1] if j >= N else U[j])
+            Hbig[r * n:(r + 1) * n, r * n:(r + 1) * n] = Uj * np.eye(n)
+            if r + 1 < tot:
+                B = bond(j)
+                Hbig[r * n:(r + 1) * n, (r + 1) * n:(r + 2) * n] = B
+                Hbig[(r + 1) * n:(r + 2) * n, r * n:(r + 1) * n] = B.conj().T
+        Gbig = np.linalg.inv(z * np.eye(tot * n) - Hbig)
+        Gdev = Gbig[L * n:(L + N) * n, L * n:(L + N) * n]
+        G, sL, sR = od.green_dense(U, ce, co, n, z, lead_kind=1)
+        assert np.max(np.abs(G - Gdev)) < 1e-9 * np.max(np.abs(Gdev))
+        # and the two self-energies on their own: Sigma = M_dev - G_dev^-1 restricted to the end blocks
+        Mdev = z * np.eye(N * n) - od.build_hamiltonian(U, ce, co, n)
+        S = Mdev - np.linalg.inv(Gdev)
+        assert np.max(np.abs(S[:n, :n] - sL)) < 1e-8 * np.max(np.abs(sL))
+        assert np.max(np.abs(S[-n:, -n:] - sR)) < 1e-8 * np.max(np.abs(sR))
+        assert np.max(np.abs(S[n:-n, n:-n])) < 1e-8            # only the end blocks carry Sigma (PAPER.md:82)
+
+
 # ------------------------------------------------------------------ P3: values printed in the paper
 
 def test_p3_paper_bandgap_and_degeneracy():
