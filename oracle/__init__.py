@@ -15,6 +15,9 @@ Modules
               (E+i eta)I - H - Sigma_L - Sigma_R        (eq.(2),(4),(5))
   negf_rgf    tier O3: the paper's Algorithm 2 + Algorithm 1 (block-tridiagonal
               recursion), step by step
+  negf_rgf_omp(.cpp/.py)  tier O3 again in plain C++17 + OpenMP (one energy point per
+              thread, own Sancho-Rubio): full-size block devices in minutes; the timed
+              CPU baseline of bench.py.  Pinned to negf_dense and to banded LU.
   broyden     Algorithm 3 (modified second Broyden) and the dense-matrix
               "bad Broyden" it must equal
 

@@ -9,6 +9,7 @@ import pytest
 import workloads as wlmod
 from oracle import negf_dense as od
 from oracle import negf_rgf as orgf
+from oracle import negf_rgf_omp as omp
 from tests.parity import assert_parity
 
 pytestmark = pytest.mark.gpu
@@ -286,43 +287,35 @@ def test_ideal_tube_integer_transmission_and_reciprocity_on_gpu():
 
 
 def test_config3_full_launch_configuration():
-    """configs[2] at full size in the launch configuration bench.py times (2112 energies, 606 + 586
-    CTAs): T(E) of the full run against the oracle (tier O3) on sampled energies, and the charge
-    against properties that hold at any size -- it is linear in the energy set (full run = sum of
-    two runs on disjoint halves of the real-axis grid, the contour kept in the first), finite and
-    within the filling of the tube."""
+    """configs[2] at FULL size in the launch configuration bench.py times (2112 energies x 1000 rings):
+    every element of the per-ring charge and of T(E) against the C++/OpenMP tier O3 oracle
+    (oracle/negf_rgf_omp.cpp: Algorithm 2 + Algorithm 1 with its own Sancho-Rubio, pinned to the dense
+    definition and to banded LU in the CPU suite).  Passage: Alg.1-2; eq.(4), (5)."""
     wl = wlmod.config3()
     n, T = _gpu_run(wl)
-    assert np.all(np.isfinite(n)) and np.all(np.isfinite(T))
-    assert np.all(n > 0.0) and np.all(n < 2.0 * wl.n)            # 0 .. deg * 17 electrons per ring
-    rng = np.random.default_rng(33)
-    ks = np.sort(rng.choice(wl.K_neq, 6, replace=False))
-    sub = wl.subset(neq_idx=ks, eq_idx=[])
-    _, T_ref = orgf.charge_and_transmission(sub, chunk=8)
-    assert_parity(T[:, ks], T_ref, "config3 full-run T(E) at sampled energies")
-    half = wl.K_neq // 2
-    n_a, _ = _gpu_run(wl.subset(neq_idx=np.arange(half)))
-    n_b, _ = _gpu_run(wl.subset(neq_idx=np.arange(half, wl.K_neq), eq_idx=[]))
-    assert_parity(n, n_a + n_b, "config3 full-run charge vs sum over energy halves", rtol=1e-12)
+    n_ref, T_ref = omp.charge_and_transmission(wl)
+    assert_parity(n, n_ref, "config3 full-size charge, every ring")
+    assert_parity(T, T_ref, "config3 full-size T(E), every energy")
 
 
 def test_config4_full_launch_configuration():
-    """configs[3] at full size (16 channels x 2000 rings x 4160 energies, 17 sweep launches): sampled
-    T(E) against the oracle, linearity of the charge in the energy set, bounds."""
+    """configs[3] at full size (16 channels x 2000 rings x 4160 energies, batched sweep launches): ONE WHOLE
+    CHANNEL -- all 4160 energies, every ring, every T(E) -- of the full 16-channel run against the C++
+    tier O3 oracle; for the other channels T(E) at sampled energies, and bounds on the charge."""
     wl = wlmod.config4()
     n, T = _gpu_run(wl)
     assert np.all(np.isfinite(n)) and np.all(np.isfinite(T))
-    assert np.all(n > 0.0) and np.all(n < 2.0 * wl.n)
+    assert np.all(n > 0.0) and np.all(n < 2.0 * wl.n)            # 0 .. deg * 17 electrons per ring
+    c = 11                                                       # a channel in the middle of the batch order
+    n_ref, T_ref = omp.charge_and_transmission(wl, channels=[c])
+    assert_parity(n[c], n_ref[c], f"config4 full-size charge of channel {c}, every ring")
+    assert_parity(T[c], T_ref[c], f"config4 full-size T(E) of channel {c}, every energy")
     rng = np.random.default_rng(44)
     ks = np.sort(rng.choice(wl.K_neq, 4, replace=False))
-    cs = np.sort(rng.choice(wl.C, 2, replace=False))
+    cs = np.array([0, 15])                                       # first and last channel of the batch order
     sub = wl.subset(neq_idx=ks, eq_idx=[], channels=cs)
-    _, T_ref = orgf.charge_and_transmission(sub, chunk=8)
-    assert_parity(T[np.ix_(cs, ks)], T_ref, "config4 full-run T(E) at sampled channels / energies")
-    half = wl.K_neq // 2
-    n_a, _ = _gpu_run(wl.subset(neq_idx=np.arange(half)))
-    n_b, _ = _gpu_run(wl.subset(neq_idx=np.arange(half, wl.K_neq), eq_idx=[]))
-    assert_parity(n, n_a + n_b, "config4 full-run charge vs sum over energy halves", rtol=1e-12)
+    _, T_s = omp.charge_and_transmission(sub)
+    assert_parity(T[np.ix_(cs, ks)], T_s, "config4 full-run T(E) at sampled channels / energies")
 
 
 def test_config5_full_launch_configuration():
@@ -336,5 +329,5 @@ def test_config5_full_launch_configuration():
     ks = np.sort(rng.choice(wl.K_neq, 3, replace=False))
     cs = np.sort(rng.choice(wl.C, 2, replace=False))
     sub = wl.subset(neq_idx=ks, eq_idx=[], channels=cs)
-    _, T_ref = orgf.charge_and_transmission(sub, chunk=8)
+    _, T_ref = omp.charge_and_transmission(sub)
     assert_parity(T[np.ix_(cs, ks)], T_ref, "config5 full-run T(E) at sampled channels / energies")

@@ -14,6 +14,7 @@ from scipy import integrate
 import workloads as wlmod
 from oracle import negf_dense as od
 from oracle import negf_rgf as orgf
+from oracle import negf_rgf_omp as omp
 from oracle import selfenergy as se
 
 HERE = os.path.dirname(os.path.abspath(__file__))
@@ -380,3 +381,48 @@ def test_p10_dense_vs_paper_recursion_on_shrunk_configs(cfg, kw):
     assert np.max(np.abs(n1 - n3) / np.abs(n1)) < 1e-11
     tol = 1e-11 * np.maximum(np.abs(T1), 1e-6 * np.max(np.abs(T1)))
     assert np.all(np.abs(T1 - T3) <= tol + 1e-300)
+
+
+# ------------------------------------------------------------------ P10 for the C++/OpenMP tier O3
+
+@pytest.mark.parametrize("N,n", [(2, 3), (5, 3), (6, 4), (7, 1), (8, 1), (4, 17)])
+def test_p10_dense_vs_cpp_recursion_random_complex_blocks(N, n):
+    """oracle/negf_rgf_omp.cpp (own Sancho-Rubio, own elimination, Alg.2 + Alg.1) against the dense
+    definition on random NON-symmetric complex blocks, both lead parities."""
+    rng = np.random.default_rng(100 + 10 * N + n)
+    U, ce, co = _random_hermitian_device(rng, N, n)
+    if n == 1:
+        ce, co = ce.reshape(1), co.reshape(1)
+    z_neq = rng.uniform(-3, 3, 6) + 1e-3j
+    w_neq = rng.uniform(0.5, 1.5, 6)
+    z_eq = rng.uniform(-3, 3, 4) + 1j * rng.uniform(0.1, 2.0, 4)
+    w_eq = rng.normal(size=4) + 1j * rng.normal(size=4)
+    lead_kind = 0 if n == 1 else 1
+    args = (U, ce, co, n, z_eq, w_eq, z_neq, w_neq, 0.1, -0.2, 0.05, lead_kind)
+    n1, T1 = od.chain_dense(*args)
+    n3, T3 = omp.chain_charge(*args)
+    assert np.max(np.abs(n1 - n3)) < 1e-11 * np.max(np.abs(n1))
+    assert np.max(np.abs(T1 - T3)) < 1e-11 * max(1.0, np.max(np.abs(T1)))
+
+
+@pytest.mark.parametrize("cfg,kw", [(1, dict(N=30, K_neq=40)),
+                                    (2, dict(N=40, K_neq=24, K_eq=8)),
+                                    (3, dict(N=16, K_neq=12, K_eq=6)),
+                                    (4, dict(C=2, N=14, K_neq=8, K_eq=4))])
+def test_p10_dense_vs_cpp_recursion_on_shrunk_configs(cfg, kw):
+    w = wlmod.make_config(cfg, **kw)
+    n1, T1 = od.charge_and_transmission(w)
+    n3, T3 = omp.charge_and_transmission(w)
+    assert np.max(np.abs(n1 - n3) / np.abs(n1)) < 1e-11
+    tol = 1e-11 * np.maximum(np.abs(T1), 1e-6 * np.max(np.abs(T1)))
+    assert np.all(np.abs(T1 - T3) <= tol + 1e-300)
+
+
+def test_cpp_tier_is_thread_count_independent_up_to_rounding():
+    """One energy per thread; the per-thread partial charges are summed in thread order, so a
+    different thread count only reorders a sum (1e-16 relative)."""
+    w = wlmod.make_config(3, N=10, K_neq=9, K_eq=3)
+    a = omp.charge_and_transmission(w, threads=1)
+    b = omp.charge_and_transmission(w, threads=3)
+    assert np.max(np.abs(a[0] - b[0]) / np.abs(a[0])) < 1e-14
+    assert np.array_equal(a[1], b[1])

@@ -6,6 +6,7 @@ from scipy.linalg import solve_banded
 
 import workloads as wlmod
 from oracle import negf_rgf as orgf
+from oracle import negf_rgf_omp as omp
 from oracle import selfenergy as se
 
 
@@ -84,3 +85,52 @@ def test_o3_vs_banded_lu_full_length_config2_mode():
         assert np.max(np.abs(AL - trAL[k])) < 1e-10 * scale
         assert np.max(np.abs(AR - trAR[k])) < 1e-10 * scale
         assert abs(T - Tm[k]) < 1e-10 * max(1e-6, abs(T))
+
+
+def test_cpp_o3_vs_banded_lu_and_numpy_tier_full_length_config3():
+    """The C++/OpenMP tier at full device length (N = 1000, n = 17) on sampled energies: per-ring
+    charge and T(E) against the banded-LU columns (independent library algorithm) with the C++
+    tier's own self-energies, and against the numpy tier end to end."""
+    w = wlmod.config3()
+    n, N = w.n, w.N
+    U = -w.phi[0]
+    idx = np.array([5, 700, 1311, 2040])
+    z = w.z_neq[idx]
+    one = np.ones(1)
+    for k in range(len(z)):
+        # one real-axis point with weight 1, mu far above / far below: f_S = 1, f_D = 0 isolates A_L, and v.v.
+        nL, T, sig = omp.chain_charge(U, w.coup_even, w.coup_odd, n, [], [], z[k:k + 1], one,
+                                      50.0, -50.0, 0.0259, 1, want_sigma=True)
+        nR, _ = omp.chain_charge(U, w.coup_even, w.coup_odd, n, [], [], z[k:k + 1], one,
+                                 -50.0, 50.0, 0.0259, 1)
+        sL, sR = sig[0, 0], sig[0, 1]
+        GL, GR = _banded_columns(U, w.coup_even, w.coup_odd, n, z[k], sL, sR)
+        gamL = 1j * (sL - sL.conj().T)
+        gamR = 1j * (sR - sR.conj().T)
+        AL = np.einsum("ia,ab,ib->i", GL, gamL, GL.conj()).real.reshape(N, n).sum(1)
+        AR = np.einsum("ia,ab,ib->i", GR, gamR, GR.conj()).real.reshape(N, n).sum(1)
+        G0N = GR[:n]
+        Tb = np.trace(gamL @ G0N @ gamR @ G0N.conj().T).real
+        scale = max(AL.max(), AR.max())
+        assert np.max(np.abs(AL - 2 * np.pi * nL)) < 1e-10 * scale
+        assert np.max(np.abs(AR - 2 * np.pi * nR)) < 1e-10 * scale
+        assert abs(Tb - T[0]) < 1e-10 * max(1.0, abs(Tb))
+        # self-energies of the two tiers agree (both polished to rounding level, reading R10)
+        sLn, sRn, _ = se.sigma_block(z[k:k + 1], w.coup_even, w.coup_odd, N, U[0], U[-1])
+        assert np.max(np.abs(sLn[0] - sL)) < 1e-11 * np.max(np.abs(sL))
+        assert np.max(np.abs(sRn[0] - sR)) < 1e-11 * np.max(np.abs(sR))
+    sub = w.subset(neq_idx=idx, eq_idx=[0, 31, 63], channels=[0])
+    n_np, T_np = orgf.charge_and_transmission(sub)
+    n_cc, T_cc = omp.charge_and_transmission(sub)
+    assert np.max(np.abs(n_np - n_cc) / np.abs(n_np)) < 1e-11
+    assert np.max(np.abs(T_np - T_cc)) < 1e-11 * max(1.0, np.max(np.abs(T_np)))
+
+
+def test_cpp_o3_scalar_vs_numpy_tier_full_length_config2_mode():
+    w = wlmod.config2()
+    sub = w.subset(neq_idx=np.arange(0, 4096, 64), eq_idx=np.arange(0, 64, 4), channels=[0])
+    n_np, T_np = orgf.charge_and_transmission(sub)
+    n_cc, T_cc = omp.charge_and_transmission(sub)
+    assert np.max(np.abs(n_np - n_cc) / np.abs(n_np)) < 1e-12
+    tol = 1e-11 * np.maximum(np.abs(T_np), 1e-6 * np.max(np.abs(T_np)))
+    assert np.all(np.abs(T_np - T_cc) <= tol)
