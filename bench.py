@@ -6,8 +6,12 @@
 A "step" is one pass of the whole hot path over one synthetic
 workload: negf_set_potential -> negf_charge (self-energies, RGF sweeps, energy reduction) ->
 negf_transmission -> the Poisson stand-in (harness code) -> broyden_step on the per-ring
-potential.  The default workload is BASELINE.json configs[1] (zigzag (17,0) tube in mode space:
-17 chains x 1000 rings, 4096 real-axis + 64 contour energies = 70 720 sweeps per step).
+potential.  BASELINE.json's metric is not quoted on one config, so the headline workload is the
+largest single-GPU configuration whose K timed + W warm-up steps finish within minutes:
+configs[3] (config 4: 16 real-space channels x 2000 rings x 17 x 17 blocks, 4096 real-axis + 64
+contour energies = 66 560 sweeps per step, ~2 s per step).  configs[4] (config 5) is the same
+kernels on a 4x larger array (30 s per step, 20 Broyden iterations = 10 minutes): it is measured
+here for a few iterations of its loop and reported under "per_config" together with configs 1-3.
 
 One JSON line is printed by rank 0; see DESIGN.md "Measurement" for every key.
 """
@@ -171,33 +175,36 @@ def algorithmic_flop_per_sweep(wl) -> float:
 # --------------------------------------------------------------------------- reference arm
 
 def cpu_oracle_sample(wl, budget_s: float = 20.0):
-    """Time the oracle (tier O3, as it stands) on a bounded sample of the workload.
+    """Time the oracle (tier O3 in C++/OpenMP, oracle/negf_rgf_omp.cpp, as it stands: one energy point
+    per thread, all host cores) on a bounded sample of the workload.
     Returns (sweeps_per_s, cores, sample description, seconds)."""
-    from oracle import negf_rgf
-    U = -wl.phi[0]
+    from oracle import negf_rgf_omp as omp
+    cores = omp.max_threads()
     t0 = time.perf_counter()
     sweeps = 0
     if wl.kind == "scalar":
+        # whole chains (all energies of one mode) until the budget is spent
+        U = -wl.phi[0]
         modes = 0
         for j in range(wl.n_modes):
-            negf_rgf.chain_charge(U, wl.coup_even[j:j + 1], wl.coup_odd[j:j + 1], 1, wl.z_eq, wl.w_eq,
-                                  wl.z_neq, wl.w_neq, wl.mu_s, wl.mu_d, wl.kT, 0, chunk=4096)
+            omp.chain_charge(U, wl.coup_even[j:j + 1], wl.coup_odd[j:j + 1], 1, wl.z_eq, wl.w_eq,
+                             wl.z_neq, wl.w_neq, wl.mu_s, wl.mu_d, wl.kT, 0)
             modes += 1
             sweeps += wl.K_eq + wl.K_neq
             if time.perf_counter() - t0 > budget_s:
                 break
         desc = f"channel 0, {modes} of {wl.n_modes} modes x all {wl.K_eq + wl.K_neq} energies"
     else:
-        chunk, done = 16, 0
+        # real-axis energies of channel 0 in chunks of 4 per core (incl. their Sancho-Rubio self-energies)
+        chunk, done = 4 * cores, 0
         while done < wl.K_neq and time.perf_counter() - t0 < budget_s:
             idx = np.arange(done, min(done + chunk, wl.K_neq))
             sub = wl.subset(neq_idx=idx, eq_idx=[], channels=[0])
-            negf_rgf.charge_and_transmission(sub, chunk=chunk)
+            omp.charge_and_transmission(sub)
             done += len(idx)
             sweeps += len(idx)
         desc = f"channel 0, first {done} real-axis energies of {wl.K_neq}"
     dt = time.perf_counter() - t0
-    cores = 1   # numpy elementwise / tiny batched LAPACK calls: single-threaded in practice
     return sweeps / dt, cores, desc, dt
 
 
@@ -217,13 +224,14 @@ def run_reference(args):
     value = tot_sweeps / tot_t
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "ranks_working": 1,    # n_gpus echoes the launch; the oracle runs on rank 0's host cores only
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": f"configs[{args.config - 1}] {wl.name}", "C": wl.C, "N": wl.N,
                    "block": wl.n, "n_modes": wl.n_modes, "K_neq": wl.K_neq, "K_eq": wl.K_eq},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
-                         "sample": desc + " per step (oracle/negf_rgf.py, numpy)"},
+                         "sample": desc + " per step (oracle/negf_rgf_omp.cpp, C++/OpenMP, one energy per thread)"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -232,26 +240,47 @@ def run_reference(args):
 
 # --------------------------------------------------------------------------- our arm
 
-def run_ours(args):
+def sancho_rubio_line(wl, stats, plan, steps, dfma_peak):
+    """Roofline sub-line of the Sancho-Rubio kernel ("report it as its own kernel line").
+    Algorithmic flop of the decimation as SURVEY 8(d) counts it: one inversion + six products on the
+    m x m principal layer, m = 2 n = 34, per pass = 56 m^3, times the passes actually executed (device
+    counter, summed over all (channel, energy, lead) tasks).  The kernel itself exploits the single
+    non-zero block of H01 (products are n x n): its executed count is 8 (2n)^3 + 8 * 8 n^3 = 128 n^3
+    per pass; both fractions are given.  The Newton polish passes (<= 4 per task, R10) are
+    not counted in either."""
+    launches, ms = stats.get("sancho_rubio", (0, 0.0))
+    if not launches or wl.kind != "block":
+        return None
+    passes = plan.get("sr_passes_total", 0)
+    m = 2 * wl.n
+    per_launch_ms = ms / launches
+    flop_alg = 56.0 * m ** 3 * passes
+    flop_exec = 128.0 * wl.n ** 3 * passes
+    tf_alg = flop_alg / (per_launch_ms * 1e-3) / 1e12
+    tf_exec = flop_exec / (per_launch_ms * 1e-3) / 1e12
+    return {"kernel": "sancho_rubio", "bound": "alu", "kernel_ms_per_launch": per_launch_ms,
+            "passes_total": int(passes), "tasks": int(wl.C * (wl.K_eq + wl.K_neq) * 2),
+            "max_passes": int(plan.get("max_sr_iterations", 0)),
+            "algorithmic_flop_per_launch": flop_alg, "achieved": tf_alg, "unit": "TFLOP/s",
+            "peak": dfma_peak, "frac": tf_alg / dfma_peak if dfma_peak else None,
+            "executed_flop_per_launch": flop_exec, "frac_executed": tf_exec / dfma_peak if dfma_peak else None,
+            "note": "56 m^3 per pass at m = 34 (SURVEY 8(d)); executed 128 n^3 per pass; polish passes not counted"}
+
+
+def measure(config, steps, warmup, world, dev, stream, peaks, e2e_steps=None, sample_clocks=True):
+    """W warm-up + K timed steps of one workload on this rank; returns the local record."""
     import torch
-    from paper_2407_14633_b200 import Broyden, Negf, negf_fp64_peak
+    from paper_2407_14633_b200 import Broyden, Negf
 
-    rank, world, local = dist_setup(args.gpus)
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
-    torch.cuda.set_device(local % torch.cuda.device_count())
-    dev = torch.device("cuda", torch.cuda.current_device())
-
-    wl, poisson = make_workload(args.config)
+    wl, poisson = make_workload(config)
     sweeps_per_step = wl.sweeps
-    stream = torch.cuda.current_stream()
     h = Negf.from_workload(wl, profile=True, stream=stream)
     bro = Broyden(wl.C * wl.N, history=8, zeta=0.1, stream=stream)
     phi_ext = torch.tensor(wl.phi, dtype=torch.float64, device=dev)
     r_dev = torch.tensor(poisson.r, dtype=torch.float64, device=dev)
     phi = phi_ext.clone()
     n = torch.empty((wl.C, wl.N), dtype=torch.float64, device=dev)
-    T = torch.empty((wl.C, wl.K_neq), dtype=torch.float64, device=dev)
+    T = torch.empty((wl.C, max(wl.K_neq, 1)), dtype=torch.float64, device=dev)
 
     def step():
         h.negf_set_potential(phi)                       # a0 (+ a1b for Sancho-Rubio leads)
@@ -260,13 +289,14 @@ def run_ours(args):
         phi_out = poisson.phi_out(phi_ext, n, r_dev)    # harness: Poisson stand-in
         bro.broyden_step(phi.view(-1), phi_out.view(-1), want_eps=False)   # a6
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         step()
     torch.cuda.synchronize()
     h.negf_kernel_stats(reset=True)
     dist_barrier(world)
-    sampler = ClockSampler(torch.cuda.current_device())
-    sampler.start()
+    sampler = ClockSampler(torch.cuda.current_device()) if sample_clocks else None
+    if sampler:
+        sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     # Timing rule: inputs larger than L2, or flush it.  The recursion history written and re-read by
@@ -276,7 +306,7 @@ def run_ours(args):
     if small:
         flush = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device=dev)
         local_ms = 0.0
-        for _ in range(args.steps):
+        for _ in range(steps):
             flush.zero_()
             e0.record(stream)
             step()
@@ -286,114 +316,183 @@ def run_ours(args):
         l2_note = "L2 flushed between steps (256 MB memset outside the per-step CUDA events)"
     else:
         e0.record(stream)
-        for _ in range(args.steps):
+        for _ in range(steps):
             step()
         e1.record(stream)
         torch.cuda.synchronize()
         local_ms = e0.elapsed_time(e1)
         l2_note = None
     dist_barrier(world)
-    clocks = sampler.stop()
+    clocks = sampler.stop() if sampler else None
     stats = h.negf_kernel_stats(reset=True)
-    n_final = n.cpu().numpy()
-    assert np.all(np.isfinite(n_final)), "non-finite charge in the timed loop"
+    h.negf_sync()
+    plan = h.negf_get_plan()
+    assert np.all(np.isfinite(n.cpu().numpy())), "non-finite charge in the timed loop"
 
     # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
-    phi_host = torch.tensor(wl.phi, dtype=torch.float64).pin_memory()
-    n_host = torch.empty((wl.C, wl.N), dtype=torch.float64).pin_memory()
-    T_host = torch.empty((wl.C, wl.K_neq), dtype=torch.float64).pin_memory()
-    for _ in range(max(1, min(args.warmup, 3))):
-        h.negf_solve_host(phi_host, n_host, T_host)
-    dist_barrier(world)
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e2.record(stream)
-    for _ in range(args.steps):
-        h.negf_solve_host(phi_host, n_host, T_host)
-    e3.record(stream)
-    torch.cuda.synchronize()
-    e2e_wall_ms = (time.perf_counter() - t0) * 1e3
-    e2e_local_ms = max(e2.elapsed_time(e3), e2e_wall_ms)   # host-synchronous call: wall clock bounds it
-    dist_barrier(world)
-    h.negf_kernel_stats(reset=True)
-
-    ms, units = dist_max_sum(local_ms, float(sweeps_per_step * args.steps), world, dev)
-    e2e_ms, e2e_units = dist_max_sum(e2e_local_ms, float(sweeps_per_step * args.steps), world, dev)
-    if rank != 0:
-        return
+    e2e = None
+    if e2e_steps:
+        phi_host = torch.tensor(wl.phi, dtype=torch.float64).pin_memory()
+        n_host = torch.empty((wl.C, wl.N), dtype=torch.float64).pin_memory()
+        T_host = torch.empty((wl.C, max(wl.K_neq, 1)), dtype=torch.float64).pin_memory()
+        h.negf_solve_host(phi_host, n_host, T_host)                      # one untimed call (kernels are warm)
+        dist_barrier(world)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e2.record(stream)
+        for _ in range(e2e_steps):
+            h.negf_solve_host(phi_host, n_host, T_host)
+        e3.record(stream)
+        torch.cuda.synchronize()
+        wall_ms = (time.perf_counter() - t0) * 1e3
+        e2e = {"local_ms": max(e2.elapsed_time(e3), wall_ms),   # host-synchronous call: wall clock bounds it
+               "steps": e2e_steps, "h2d": int(phi_host.numel() * 8),
+               "d2h": int((n_host.numel() + wl.C * wl.K_neq) * 8)}
+        dist_barrier(world)
+        h.negf_kernel_stats(reset=True)
 
     # ---- roofline of the dominant kernel
+    hbm_peak, peak_src, dfma, dmma = peaks
     kname = "scalar_sweep" if wl.kind == "scalar" else "block_sweep"
     launches, k_ms = stats.get(kname, (0, 0.0))
     per_launch_ms = k_ms / max(launches, 1)
-    launches_per_step = max(launches, 1) / args.steps
-    hbm_peak, peak_src = load_peaks()
+    launches_per_step = max(launches, 1) / steps
     if wl.kind == "scalar":
-        alg_bytes = algorithmic_bytes_per_sweep(wl) * sweeps_per_step / launches_per_step
-        achieved = alg_bytes / (per_launch_ms * 1e-3) / 1e9 if per_launch_ms > 0 else 0.0
+        alg = algorithmic_bytes_per_sweep(wl) * sweeps_per_step / launches_per_step
+        achieved = alg / (per_launch_ms * 1e-3) / 1e9 if per_launch_ms > 0 else 0.0
         roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
-                    "frac": achieved / hbm_peak, "traffic": load_traffic(kname, args.config),
+                    "frac": achieved / hbm_peak, "traffic": load_traffic(kname, config),
                     "kernel": kname, "kernel_ms_per_launch": per_launch_ms,
-                    "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src}
+                    "algorithmic_bytes_per_launch": alg, "peak_source": peak_src}
     else:
-        dfma, dmma = negf_fp64_peak()
-        alg_flop = algorithmic_flop_per_sweep(wl) * sweeps_per_step / launches_per_step
-        achieved = alg_flop / (per_launch_ms * 1e-3) / 1e12 if per_launch_ms > 0 else 0.0
+        alg = algorithmic_flop_per_sweep(wl) * sweeps_per_step / launches_per_step
+        achieved = alg / (per_launch_ms * 1e-3) / 1e12 if per_launch_ms > 0 else 0.0
         roofline = {"bound": "alu", "achieved": achieved, "peak": dfma, "unit": "TFLOP/s",
                     "frac": achieved / dfma if dfma > 0 else None,
-                    "traffic": load_traffic(kname, args.config), "kernel": kname,
-                    "kernel_ms_per_launch": per_launch_ms, "algorithmic_flop_per_launch": alg_flop,
+                    "traffic": load_traffic(kname, config), "kernel": kname + " (forward sweep + way back)",
+                    "kernel_ms_per_launch": per_launch_ms, "algorithmic_flop_per_launch": alg,
                     "peak_source": "FP64 DFMA chain measured live (negf_fp64_peak); DMMA: %.1f" % dmma}
-    kernel_share = {k: round(v[1] / ms, 4) for k, v in stats.items() if v[0]}
+    rec = {
+        "wl": wl, "local_ms": local_ms, "units": float(sweeps_per_step * steps), "steps": steps,
+        "sweeps_per_step": sweeps_per_step, "clocks": clocks, "stats": stats, "plan": plan,
+        "roofline": roofline, "l2_note": l2_note, "e2e": e2e,
+        "sancho_rubio": sancho_rubio_line(wl, stats, plan, steps, dfma),
+        "launches_per_step": plan["kernel_launches"] + 4,     # + 4 Broyden kernels
+    }
+    h.negf_destroy()
+    bro.broyden_destroy()
+    del phi, phi_ext, n, T
+    torch.cuda.empty_cache()
+    return rec
+
+
+# timed steps / warm-ups of the per_config legs (bounded so that the default run finishes within minutes)
+PER_CONFIG_STEPS = {1: (50, 3), 2: (50, 3), 3: (5, 3), 4: (3, 3), 5: (2, 3)}
+
+
+def run_ours(args):
+    import torch
+    from paper_2407_14633_b200 import negf_fp64_peak
+
+    rank, world, local = dist_setup(args.gpus)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    torch.cuda.set_device(local % torch.cuda.device_count())
+    dev = torch.device("cuda", torch.cuda.current_device())
+    stream = torch.cuda.current_stream()
+    hbm_peak, peak_src = load_peaks()
+    dfma, dmma = negf_fp64_peak()
+    peaks = (hbm_peak, peak_src, dfma, dmma)
+
+    # ---- headline workload
+    block = args.config >= 3
+    e2e_steps = min(args.steps, 3) if block else args.steps
+    rec = measure(args.config, args.steps, args.warmup, world, dev, stream, peaks, e2e_steps=e2e_steps)
+    wl = rec["wl"]
+    ms, units = dist_max_sum(rec["local_ms"], rec["units"], world, dev)
+    e2e_ms, e2e_units = dist_max_sum(rec["e2e"]["local_ms"], float(rec["sweeps_per_step"] * rec["e2e"]["steps"]),
+                                     world, dev)
+
+    # ---- the other configs, same run (rank 0 reports; every rank runs them so that the replicas stay in step)
+    per_config = {}
+    if args.per_config != "none":
+        wanted = [int(c) for c in args.per_config.split(",")] if args.per_config != "all" else [1, 2, 3, 4, 5]
+        for c in wanted:
+            if c == args.config:
+                continue
+            k, w = PER_CONFIG_STEPS[c]
+            r = measure(c, k, w, world, dev, stream, peaks, e2e_steps=None, sample_clocks=False)
+            cms, cunits = dist_max_sum(r["local_ms"], r["units"], world, dev)
+            entry = {
+                "workload": f"configs[{c - 1}] {r['wl'].name}", "value": cunits / (cms * 1e-3), "unit": UNIT,
+                "steps": k, "warmup": w, "ms_per_step": cms / k, "sweeps_per_step": r["sweeps_per_step"],
+                "roofline": {kk: r["roofline"][kk] for kk in ("bound", "achieved", "peak", "unit", "frac", "kernel",
+                                                               "kernel_ms_per_launch", "traffic")},
+                "kernel_share_of_step": {kk: round(v[1] / r["local_ms"], 4) for kk, v in r["stats"].items() if v[0]},
+            }
+            if r["sancho_rubio"]:
+                entry["sancho_rubio"] = {kk: r["sancho_rubio"][kk] for kk in ("frac", "frac_executed", "achieved",
+                                                                             "kernel_ms_per_launch", "passes_total")}
+            if c == 1:
+                entry["note"] = "1000 sweeps of 100 sites: launch-latency-bound (SURVEY 8(d)); parity / smoke config"
+            if c == 5:
+                entry["note"] = ("one step = one Broyden iteration of the 20-iteration loop (history 8, mixing 0.1); "
+                                 "the full loop is 20 x ms_per_step")
+            per_config[f"config{c}"] = entry
+    if rank != 0:
+        return
 
     cpu_baseline = None
     if world == 1:
         cpu_sps, cores, desc, cpu_dt = cpu_oracle_sample(wl, budget_s=args.cpu_budget)
         cpu_baseline = {"value": cpu_sps, "unit": UNIT, "cores": cores, "kind": "oracle",
-                        "sample": desc + f" ({cpu_dt:.1f} s, oracle/negf_rgf.py)"}
+                        "sample": desc + f" ({cpu_dt:.1f} s, oracle/negf_rgf_omp.cpp, C++/OpenMP, one energy per thread)"}
 
-    # my kernels per step: negf_set_potential + negf_charge (counted by the library's plan) + 4 Broyden
-    plan = h.negf_get_plan()
-    my_launches = args.steps * (plan["kernel_launches"] + 4)
     value = units / (ms * 1e-3)
+    plan = rec["plan"]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"configs[{args.config - 1}] {wl.name}", "C": wl.C, "N": wl.N,
                    "block": wl.n, "n_modes": wl.n_modes, "K_neq": wl.K_neq, "K_eq": wl.K_eq,
-                   "sweeps_per_step": sweeps_per_step, "parallelism": f"replicas x{world}",
-                   "l2": l2_note or "recursion history %.2f GB per step >> 126 MB L2 (no flush needed)" % (
+                   "sweeps_per_step": rec["sweeps_per_step"], "parallelism": f"replicas x{world}",
+                   "l2": rec["l2_note"] or "recursion history %.2f GB per step >> 126 MB L2 (no flush needed)" % (
                        plan["history_bytes"] / 1e9),
                    "step": "set_potential+charge+transmission+poisson_stand_in+broyden_step"},
-        "clocks": clocks,
+        "clocks": rec["clocks"],
         "e2e": {"value": e2e_units / (e2e_ms * 1e-3), "unit": UNIT,
-                "h2d_bytes_per_step": int(phi_host.numel() * 8),
-                "d2h_bytes_per_step": int((n_host.numel() + T_host.numel()) * 8),
-                "ms_per_step": e2e_ms / args.steps, "call": "negf_solve_host (pinned host buffers)"},
-        "gpu_launches": int(my_launches),
-        "roofline": roofline,
-        "kernel_share_of_step": kernel_share,
+                "h2d_bytes_per_step": rec["e2e"]["h2d"], "d2h_bytes_per_step": rec["e2e"]["d2h"],
+                "ms_per_step": e2e_ms / rec["e2e"]["steps"], "steps": rec["e2e"]["steps"],
+                "call": "negf_solve_host (pinned host buffers)",
+                "covers": "H2D of phi + negf_set_potential + negf_charge + T(E) + D2H of n and T; the Poisson "
+                          "stand-in (harness) and broyden_step of `value`'s step are not part of this call"},
+        "gpu_launches": int(args.steps * rec["launches_per_step"]),
+        "roofline": rec["roofline"],
+        "sancho_rubio": rec["sancho_rubio"],
+        "kernel_share_of_step": {k: round(v[1] / rec["local_ms"], 4) for k, v in rec["stats"].items() if v[0]},
+        "per_config": per_config,
         "cpu_baseline": cpu_baseline,
     }
     print(json.dumps(line), flush=True)
-    h.negf_destroy()
-    bro.broyden_destroy()
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=None,
-                    help="timed steps (default: 200 for the scalar configs, whose step is ~0.6 ms; 5 for config 3; 2 for configs 4-5)")
+                    help="timed steps of the headline workload (default: 5 for config 4; 200 for the scalar "
+                         "configs, whose step is ~0.6 ms; 5 for config 3; 2 for config 5)")
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config, 1-based")
+    ap.add_argument("--config", type=int, default=4, help="headline BASELINE.json config, 1-based")
+    ap.add_argument("--per-config", default="all", dest="per_config",
+                    help="other configs measured in the same run: 'all', 'none' or e.g. '2,3'")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-budget", type=float, default=15.0, dest="cpu_budget")
     args = ap.parse_args()
     if args.steps is None:
-        args.steps = {1: 200, 2: 200, 3: 5}.get(args.config, 2) if args.impl == "ours" else 3
+        args.steps = {1: 200, 2: 200, 3: 5, 4: 5}.get(args.config, 2) if args.impl == "ours" else 3
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3            # timing rule: W >= 3
     if args.impl == "reference":

@@ -65,11 +65,14 @@ typedef struct broyden_handle broyden_handle; /* opaque */
 typedef struct {
   int32_t n_channels;  /* C >= 1: independent channels batched together                 */
   int32_t n_rings;     /* N >= 2: rings per channel, the same for every channel of a handle             */
-  int32_t block;       /* n: 1 = scalar mode-space chains, > 1 = dense n x n blocks (<= 32; 17 for (17,0)) */
+  int32_t block;       /* n: 1 = scalar mode-space chains, > 1 = dense n x n blocks.  The block kernels are
+                          instantiated for n in {2, 3, 4, 5, 8, 17} (17 = the (17,0) tube); any other n > 1
+                          returns NEGF_EINVAL                                                              */
   int32_t n_modes;     /* block == 1: chains (modes) per channel; block > 1: must be 1    */
   int32_t lead_kind;   /* 0 = closed-form alternating chain (block == 1 only); 1 = Sancho-Rubio (block > 1) */
   int32_t sr_maxit;    /* lead_kind 1: iteration cap (200)                                               */
-  double  sr_tol;      /* lead_kind 1: stop when max|a_ij|,|b_ij| < sr_tol (1e-12), then one more pass (R10) */
+  double  sr_tol;      /* lead_kind 1: stop when max|a_ij|,|b_ij| < sr_tol (1e-12), then two more passes and the
+                          Newton polish of the fixed point (R10)                                           */
   double  mu_s, mu_d;  /* eV: electrochemical potentials of the source (left, ring 0) and drain leads    */
   double  kT;          /* eV, > 0                                                                        */
   double  deg;         /* degeneracy prefactor of eq.(3), PAPER.md:86 (g_s = 2)                          */
@@ -82,10 +85,18 @@ typedef struct {
   int32_t n_neq;              /* K_neq >= 0 real-axis points (eq.(4) second term)                        */
   const negf_c64* z_neq;      /* nodes E_k + i eta (the caller supplies eta, R11)                        */
   const double*   w_neq;      /* real quadrature weights; Fermi factors are applied by the library       */
-  int64_t workspace_bytes;    /* cap on the recursion-history workspace in HBM; 0 = default (64 GiB).
+  int64_t workspace_bytes;    /* cap on the recursion-history workspace in HBM.  0 = default: what the plan
+                                 needs, at most 64 GiB (block == 1) or, for block > 1, at most two waves of
+                                 resident sweep CTAs and 85 % of the FREE device memory at creation -- two
+                                 full-size block handles do not fit one GPU unless both pass a cap here.
                                  Larger problems are tiled over (channel, energy) batches. */
   int32_t profile;            /* != 0: record CUDA events around every kernel (negf_kernel_stats)        */
-  int32_t reserved;
+  int32_t reserved;           /* must be 0                                                               */
+  double  pivot_theta;        /* block > 1: the diagonal pivot candidate of an in-register Gauss-Jordan step is
+                                 accepted without a search when |a_kk| >= theta * ||row k of the matrix handed
+                                 in||_2; otherwise the task searches the whole column (partial pivoting).
+                                 0 = default (1e-3); a huge value (1e150) forces the search at every
+                                 elimination step (test hook).                                             */
 } negf_config;
 
 /* Create a handle: validates, copies the config, allocates workspace.  `cuda_stream` is a
@@ -125,8 +136,9 @@ NEGF_API negf_status negf_current(negf_handle* h, double* current_dev, double* c
  * memory and synchronises the stream. */
 NEGF_API negf_status negf_solve_host(negf_handle* h, const double* phi_host, double* n_host, double* T_host);
 
-/* Block until the handle's stream is idle; returns NEGF_ENOCONV / NEGF_ECUDA if something went wrong
- * on the device since the last sync. */
+/* Block until the handle's stream is idle; returns NEGF_ENOCONV if a Sancho-Rubio task of any
+ * negf_set_potential since the last negf_sync / negf_solve_host did not converge (the flag is sticky
+ * until it has been reported once), NEGF_ECUDA if the device reported an error. */
 NEGF_API negf_status negf_sync(negf_handle* h);
 
 /* Per-kernel timing (only when cfg.profile != 0).  Synchronises.  Fills up to *count entries. */
@@ -145,6 +157,8 @@ typedef struct {
   int32_t sweeps_per_charge; /* C * chains * (K_eq + K_neq)                              */
   int32_t max_sr_iterations; /* largest Sancho-Rubio iteration count of the last set_potential (after sync) */
   int32_t kernel_launches;   /* kernels launched by one negf_set_potential + negf_charge pair               */
+  int64_t sr_passes_total;   /* decimation passes of the last negf_set_potential summed over all
+                                (channel, energy, lead) tasks (after sync)                                  */
 } negf_plan_info;
 NEGF_API negf_status negf_get_plan(negf_handle* h, negf_plan_info* out);
 
@@ -164,13 +178,6 @@ NEGF_API negf_status broyden_destroy(broyden_handle* h);
  * DFMA instructions and of DMMA (mma.sync.m8n8k4.f64) instructions; used as the roofline denominator
  * of the FP64-bound block kernels.  Synchronous; takes a few milliseconds. */
 NEGF_API negf_status negf_fp64_peak(double* dfma_tflops, double* dmma_tflops);
-
-/* Diagnostic / test hook of the block path's in-register Gauss-Jordan inversion: a diagonal pivot
- * candidate is accepted when |a_kk| >= theta * ||row k of the matrix handed in||_2, otherwise the task
- * searches the whole column (partial pivoting).  theta <= 0 restores the default (1e-3); a huge theta
- * (e.g. 1e150) forces the search at every elimination step.  Process-wide; affects kernels launched
- * afterwards. */
-NEGF_API negf_status negf_set_pivot_threshold(double theta);
 
 /* Last error text of the calling thread (static storage, never NULL). */
 NEGF_API const char* negf_last_error(void);

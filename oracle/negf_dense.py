@@ -147,3 +147,49 @@ def green_dense(U, coup_even, coup_odd, n, z, lead_kind=0, sr_tol=1e-12, sr_maxi
     M[:n, :n] -= sL[0]
     M[D - n:, D - n:] -= sR[0]
     return np.linalg.inv(M), sL[0], sR[0]
+
+
+def landauer_dense(wl, channels=None):
+    """Lead currents and zero-bias conductance BY DEFINITION (eq.(5)-(6)), from the
+    dense Green's function -- not from T(E):
+
+      I_l = (g_s e/h) int Tr[ F_l Gamma_l A + i Gamma_l G^< ] dE,   A = sum_l A_l,  G^< = i sum_l A_l F_l
+      G   = G_0 int T(E) (-dF/dE) dE,   T = Tr[Gamma_S G^R Gamma_D G^R^dagger],  F = F(E - mu_S, kT)
+
+    on the real-axis nodes / weights of the workload.  Returns (I_S[C], I_D[C], G[C]) with the
+    currents in eV (multiply by g_s e/h) and G in units of G_0; scalar chains are summed over modes
+    with ``mode_weight``.  For two leads the integrand of I_S reduces algebraically to
+    T_SD (F_S - F_D); this function does not use that."""
+    chans = range(wl.C) if channels is None else channels
+    I_S = np.zeros(wl.C)
+    I_D = np.zeros(wl.C)
+    G = np.zeros(wl.C)
+    E = wl.z_neq.real
+    fS = fermi_real(E, wl.mu_s, wl.kT)
+    fD = fermi_real(E, wl.mu_d, wl.kT)
+    dfdE = fS * (1.0 - fS) / wl.kT                      # -dF/dE of the source Fermi function
+    for c in chans:
+        U = -wl.phi[c]
+        units = ([(wl.coup_even[j:j + 1], wl.coup_odd[j:j + 1], 1, 0, wl.mode_weight[j])
+                  for j in range(wl.n_modes)] if wl.kind == "scalar"
+                 else [(wl.coup_even, wl.coup_odd, wl.n, 1, 1.0)])
+        for ce, co, n, lead_kind, wgt in units:
+            N = U.shape[0]
+            D = N * n
+            for k, z in enumerate(wl.z_neq):
+                Gr, sL, sR = green_dense(U, ce, co, n, z, lead_kind, wl.sr_tol, wl.sr_maxit)
+                gamL = np.zeros((D, D), dtype=np.complex128)
+                gamR = np.zeros((D, D), dtype=np.complex128)
+                gamL[:n, :n] = 1j * (sL - sL.conj().T)
+                gamR[D - n:, D - n:] = 1j * (sR - sR.conj().T)
+                AL = Gr @ gamL @ Gr.conj().T
+                AR = Gr @ gamR @ Gr.conj().T
+                A = AL + AR
+                Gless = 1j * (AL * fS[k] + AR * fD[k])
+                iS = np.trace(fS[k] * gamL @ A + 1j * gamL @ Gless).real
+                iD = np.trace(fD[k] * gamR @ A + 1j * gamR @ Gless).real
+                T = np.trace(gamL @ Gr @ gamR @ Gr.conj().T).real
+                I_S[c] += wgt * wl.w_neq[k] * iS
+                I_D[c] += wgt * wl.w_neq[k] * iD
+                G[c] += wgt * wl.w_neq[k] * T * dfdE[k]
+    return I_S, I_D, G

@@ -12,6 +12,5 @@ from .binding import (  # noqa: F401
     EXPORTED_SYMBOLS,
     load_library,
     negf_fp64_peak,
-    negf_set_pivot_threshold,
     negf_version,
 )

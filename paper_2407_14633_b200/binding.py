@@ -27,7 +27,7 @@ EXPORTED_SYMBOLS = [
     "negf_create", "negf_destroy", "negf_set_potential", "negf_charge", "negf_transmission",
     "negf_self_energy", "negf_current", "negf_solve_host", "negf_sync", "negf_kernel_stats", "negf_get_plan",
     "broyden_create", "broyden_step", "broyden_reset", "broyden_destroy",
-    "negf_fp64_peak", "negf_set_pivot_threshold", "negf_last_error", "negf_version",
+    "negf_fp64_peak", "negf_last_error", "negf_version",
 ]
 
 
@@ -51,6 +51,7 @@ class negf_config(C.Structure):
         ("n_eq", C.c_int32), ("z_eq", C.c_void_p), ("w_eq", C.c_void_p),
         ("n_neq", C.c_int32), ("z_neq", C.c_void_p), ("w_neq", C.c_void_p),
         ("workspace_bytes", C.c_int64), ("profile", C.c_int32), ("reserved", C.c_int32),
+        ("pivot_theta", C.c_double),
     ]
 
 
@@ -61,7 +62,8 @@ class negf_kernel_stat(C.Structure):
 class negf_plan_info(C.Structure):
     _fields_ = [("history_bytes", C.c_int64), ("partial_bytes", C.c_int64),
                 ("n_batches", C.c_int32), ("sweeps_per_charge", C.c_int32),
-                ("max_sr_iterations", C.c_int32), ("kernel_launches", C.c_int32)]
+                ("max_sr_iterations", C.c_int32), ("kernel_launches", C.c_int32),
+                ("sr_passes_total", C.c_int64)]
 
 
 _lib = None
@@ -96,7 +98,6 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
         "broyden_reset": (C.c_int, [vp]),
         "broyden_destroy": (C.c_int, [vp]),
         "negf_fp64_peak": (C.c_int, [C.POINTER(dbl), C.POINTER(dbl)]),
-        "negf_set_pivot_threshold": (C.c_int, [dbl]),
         "negf_last_error": (C.c_char_p, []),
         "negf_version": (C.c_char_p, []),
     }
@@ -148,7 +149,7 @@ class Negf:
     def __init__(self, *, n_channels, n_rings, block, n_modes, lead_kind, coup_even, coup_odd,
                  mode_weight=None, z_eq=None, w_eq=None, z_neq=None, w_neq=None,
                  mu_s=0.0, mu_d=0.0, kT=0.0259, deg=2.0, sr_tol=1e-12, sr_maxit=200,
-                 workspace_bytes=0, profile=False, stream=None):
+                 workspace_bytes=0, profile=False, pivot_theta=0.0, stream=None):
         self._lib = load_library()
         self._h = C.c_void_p(None)
         keep = []
@@ -177,7 +178,7 @@ class Negf:
             deg=deg, coup_even=_ptr(ce), coup_odd=_ptr(co), mode_weight=_ptr(mw),
             n_eq=ze.size, z_eq=_ptr(ze), w_eq=_ptr(we), n_neq=zn.size, z_neq=_ptr(zn),
             w_neq=_ptr(wn), workspace_bytes=int(workspace_bytes), profile=int(bool(profile)),
-            reserved=0)
+            reserved=0, pivot_theta=float(pivot_theta))
         self.C, self.N, self.K_neq = int(n_channels), int(n_rings), int(zn.size)
         _check(self._lib.negf_create(C.byref(cfg), _stream_ptr(stream), C.byref(self._h)),
                "negf_create")
@@ -303,10 +304,6 @@ def negf_fp64_peak():
     a, b = C.c_double(0.0), C.c_double(0.0)
     _check(load_library().negf_fp64_peak(C.byref(a), C.byref(b)), "negf_fp64_peak")
     return a.value, b.value
-
-
-def negf_set_pivot_threshold(theta: float) -> None:
-    _check(load_library().negf_set_pivot_threshold(float(theta)), "negf_set_pivot_threshold")
 
 
 def negf_version() -> str:

@@ -49,7 +49,7 @@ struct CtaId17 {
 };
 // real-axis CTA numbering of block_sweep.cu: after the C*geq*2 contour CTAs, (channel, group, direction)
 __device__ __forceinline__ CtaId17 decode_real_cta(const SweepLaunch& p, long long gid) {
-  const long long r = gid - (long long)p.C * p.geq * 2;
+  const long long r = gid - p.n_eq_cta;
   const int per = 2 * p.gneq;
   CtaId17 id;
   id.c = (int)(r / per);
@@ -64,6 +64,7 @@ __device__ __forceinline__ CtaId17 decode_real_cta(const SweepLaunch& p, long lo
 __global__ void __launch_bounds__(kBackThreads17, 2) block_back17_kernel(const SweepLaunch p, long long first_gid) {
   using G = Geo2<NB17>;
   constexpr int TPC = G::TPC;                       // 7 tasks = 7 warps
+  constexpr long long STEP = G::STEP_ELEMS;
   constexpr int MAT = NB17 * NB17;
   __shared__ __align__(16) c64 Bs_all[TPC][NB17 * LDB];
   __shared__ double red[TPC][32];
@@ -91,13 +92,13 @@ __global__ void __launch_bounds__(kBackThreads17, 2) block_back17_kernel(const S
 
   c64* Bs = Bs_all[t];
   for (int e = lane; e < MAT; e += 32) Bs[(e / NB17) * LDB + (e % NB17)] = F_last[e];   // C_N := F_k
-  const c64* hrec = p.hist + (slot * (size_t)N + (N - 1)) * G::STEP_ELEMS + (size_t)t * kHistRec17;
+  const c64* hrec = p.hist + (slot * (size_t)N + (N - 1)) * STEP + (size_t)t * kHistRec17;
   const int off_frag = g * kHistLd17 + q4;                               // + mt*8*18 + ks*4
   const int off_bord = lane < 16 ? lane * kHistLd17 + 16 : 16 * kHistLd17 + (lane - 16);
 
   double keep = 0.0;
   int cnt = 0;                                       // rings done; ring N-1-cnt is next
-  for (int s = N - 1; s >= 0; --s, hrec -= G::STEP_ELEMS, ++cnt) {
+  for (int s = N - 1; s >= 0; --s, hrec -= STEP, ++cnt) {
     // ---- operands of this ring: A fragments and border of ytilde_s
     c64 Ar[2][4];
 #pragma unroll
@@ -107,7 +108,7 @@ __global__ void __launch_bounds__(kBackThreads17, 2) block_back17_kernel(const S
     const c64 bord = hrec[off_bord];                 // lane l < 16: ytilde[l][16]; lane 16+j: ytilde[16][j]
     const c64 acorner = hrec[16 * kHistLd17 + 16];   // ytilde[16][16]
     if (s > 0) {                                     // next ring's 39 lines towards L2
-      const char* nx = reinterpret_cast<const char*>(hrec - G::STEP_ELEMS);
+      const char* nx = reinterpret_cast<const char*>(hrec - STEP);
       asm volatile("prefetch.global.L2 [%0];" ::"l"(nx + 128 * lane));
       if (lane < 7) asm volatile("prefetch.global.L2 [%0];" ::"l"(nx + 128 * (32 + lane)));
     }
@@ -235,8 +236,7 @@ __global__ void __launch_bounds__(kBackThreads17, 2) block_back17_kernel(const S
 
 cudaError_t launch_block_back17(const SweepLaunch& p, cudaStream_t s) {
   // real-axis CTAs of this launch: global ids [max(cta_begin, n_eq_cta), cta_begin + n_cta)
-  const long long n_eq_cta = (long long)p.C * p.geq * 2;
-  const long long first = p.cta_begin > n_eq_cta ? p.cta_begin : n_eq_cta;
+  const long long first = p.cta_begin > p.n_eq_cta ? p.cta_begin : p.n_eq_cta;
   const long long n = p.cta_begin + p.n_cta - first;
   if (n <= 0) return cudaSuccess;
   block_back17_kernel<<<(unsigned)n, kBackThreads17, 0, s>>>(p, first);

@@ -23,6 +23,7 @@ struct BlockPath {
   int sr_maxit;
   const double2 *z_eq, *w_eq, *z_neq;   // owned by the negf_handle
   const double* w_neq;
+  double theta2;        // pivot acceptance threshold squared (negf_config.pivot_theta)
   // geometry
   int tpc, threads, geq, gneq;
   long long total_cta, n_eq_cta;
@@ -41,13 +42,10 @@ struct BlockPath {
   double* partial;
   double* scratch;
   int* flags;       // [0] max SR iterations, [1] non-convergence flag
+  unsigned long long* counters;   // [0] Sancho-Rubio passes of the last set_potential, summed over all tasks
   int last_max_iters;
+  long long last_sr_passes;
 };
-
-static double g_theta2 = blk::kTheta2Default;
-void block_path_set_pivot_threshold(double theta) {
-  g_theta2 = theta > 0.0 ? theta * theta : blk::kTheta2Default;
-}
 
 namespace {
 
@@ -88,7 +86,7 @@ void block_path_destroy(BlockPath* bp) {
   if (!bp) return;
   cudaFree(bp->csr_rowptr); cudaFree(bp->csr_col); cudaFree(bp->csr_val); cudaFree(bp->csr_diag);
   cudaFree(bp->lead_mats); cudaFree(bp->table); cudaFree(bp->hist);
-  cudaFree(bp->partial); cudaFree(bp->scratch); cudaFree(bp->flags);
+  cudaFree(bp->partial); cudaFree(bp->scratch); cudaFree(bp->flags); cudaFree(bp->counters);
   delete bp;
 }
 
@@ -108,6 +106,7 @@ negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, c
   bp->K_eq = cfg->n_eq; bp->K_neq = cfg->n_neq;
   bp->mu_s = cfg->mu_s; bp->mu_d = cfg->mu_d; bp->kT = cfg->kT; bp->deg = cfg->deg;
   bp->sr_tol = cfg->sr_tol; bp->sr_maxit = cfg->sr_maxit;
+  bp->theta2 = cfg->pivot_theta > 0.0 ? cfg->pivot_theta * cfg->pivot_theta : blk::kTheta2Default;
   bp->z_eq = z_eq_dev; bp->w_eq = w_eq_dev; bp->z_neq = z_neq_dev; bp->w_neq = w_neq_dev;
   auto fail = [&](negf_status st) { block_path_destroy(bp); return st; };
 
@@ -210,6 +209,8 @@ negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, c
   chk(cudaMalloc((void**)&bp->scratch, sizeof(double) * (size_t)bp->C * nslice * bp->N));
   chk(cudaMalloc((void**)&bp->flags, 2 * sizeof(int)));
   if (e == cudaSuccess) chk(cudaMemset(bp->flags, 0, 2 * sizeof(int)));
+  chk(cudaMalloc((void**)&bp->counters, sizeof(unsigned long long)));
+  if (e == cudaSuccess) chk(cudaMemset(bp->counters, 0, sizeof(unsigned long long)));
   if (e != cudaSuccess) {
     set_error("negf_create (block path): device allocation failed: %s", cudaGetErrorString(e));
     return fail(e == cudaErrorMemoryAllocation ? NEGF_ENOMEM : NEGF_ECUDA);
@@ -227,6 +228,8 @@ negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, c
   bp->slot_bytes = (int64_t)sizeof(double2) * bp->N * blk::block_step_elems(n);
   size_t free_b = 0, total_b = 0;
   cudaMemGetInfo(&free_b, &total_b);
+  // default (workspace_bytes = 0): what two waves of resident CTAs need, never more than 85 % of the free
+  // device memory (include/negf.h)
   int64_t budget = cfg->workspace_bytes > 0 ? cfg->workspace_bytes : (int64_t)((double)free_b * 0.85);
   budget = std::min<int64_t>(budget, (int64_t)((double)free_b * 0.95));
   long long slots = std::min<long long>(bp->total_cta, budget / bp->slot_bytes);
@@ -256,9 +259,12 @@ negf_status block_path_self_energy(BlockPath* bp, const double* U_dev, cudaStrea
   p.C = bp->C; p.N = bp->N; p.K_eq = bp->K_eq; p.K_neq = bp->K_neq;
   p.U = U_dev; p.z_eq = bp->z_eq; p.z_neq = bp->z_neq;
   p.lead_mats = bp->lead_mats; p.table = bp->table;
-  p.tol = bp->sr_tol; p.shift = bp->sr_shift; p.maxit = bp->sr_maxit; p.theta2 = g_theta2;
-  p.max_iters = bp->flags; p.noconv_flag = bp->flags + 1;
-  NEGF_CUDA_TRY(cudaMemsetAsync(bp->flags, 0, 2 * sizeof(int), s));
+  p.tol = bp->sr_tol; p.shift = bp->sr_shift; p.maxit = bp->sr_maxit; p.theta2 = bp->theta2;
+  p.max_iters = bp->flags; p.noconv_flag = bp->flags + 1; p.iters_total = bp->counters;
+  NEGF_CUDA_TRY(cudaMemsetAsync(bp->counters, 0, sizeof(unsigned long long), s));
+  // [0] = largest iteration count of THIS call; [1] = non-convergence flag, sticky until block_path_check
+  // has reported it (a Broyden loop that never syncs in between must not lose it)
+  NEGF_CUDA_TRY(cudaMemsetAsync(bp->flags, 0, sizeof(int), s));
   hook.begin(hook.ctx, 0);
   cudaError_t e = blk::launch_sancho_rubio(bp->n, p, s);
   hook.end(hook.ctx);
@@ -270,10 +276,10 @@ negf_status block_path_run(BlockPath* bp, const double* U_dev, double* n_res, do
                            cudaStream_t s, ProfHook hook) {
   blk::SweepLaunch p;
   p.C = bp->C; p.N = bp->N; p.K_eq = bp->K_eq; p.K_neq = bp->K_neq;
-  p.geq = bp->geq; p.gneq = bp->gneq;
+  p.geq = bp->geq; p.gneq = bp->gneq; p.n_eq_cta = bp->n_eq_cta;
   p.U = U_dev; p.z_eq = bp->z_eq; p.w_eq = bp->w_eq; p.z_neq = bp->z_neq; p.w_neq = bp->w_neq;
   p.table = bp->table;
-  p.mu_s = bp->mu_s; p.mu_d = bp->mu_d; p.kT = bp->kT; p.deg = bp->deg; p.theta2 = g_theta2;
+  p.mu_s = bp->mu_s; p.mu_d = bp->mu_d; p.kT = bp->kT; p.deg = bp->deg; p.theta2 = bp->theta2;
   p.hist = bp->hist; p.partial = bp->partial; p.T = T_res;
   p.csr.rowptr = bp->csr_rowptr; p.csr.col = bp->csr_col; p.csr.val = bp->csr_val;
   p.csr.nnz_cap = bp->nnz_cap;
@@ -314,7 +320,11 @@ negf_status block_path_check(BlockPath* bp) {
   int host[2] = {0, 0};
   NEGF_CUDA_TRY(cudaMemcpy(host, bp->flags, sizeof(host), cudaMemcpyDeviceToHost));
   bp->last_max_iters = host[0];
+  unsigned long long cnt = 0;
+  NEGF_CUDA_TRY(cudaMemcpy(&cnt, bp->counters, sizeof(cnt), cudaMemcpyDeviceToHost));
+  bp->last_sr_passes = (long long)cnt;
   if (host[1]) {
+    NEGF_CUDA_TRY(cudaMemset(bp->flags + 1, 0, sizeof(int)));
     set_error("Sancho-Rubio decimation did not reach sr_tol within sr_maxit = %d iterations for at least "
               "one (channel, energy, lead)", bp->sr_maxit);
     return NEGF_ENOCONV;
@@ -327,10 +337,15 @@ void block_path_plan(BlockPath* bp, negf_plan_info* out) {
   out->partial_bytes = bp->partial_bytes;
   out->n_batches = bp->n_launches;
   out->max_sr_iterations = bp->last_max_iters;
-  // negate + Sancho-Rubio + sweep launches + one combine per launch that holds contour CTAs + 2-level reduce
-  int combines = 0;
-  for (long long begin = 0; begin < bp->n_eq_cta; begin += bp->slots) ++combines;
-  out->kernel_launches = 1 + 1 + bp->n_launches + combines + 2;
+  out->sr_passes_total = bp->last_sr_passes;
+  // negate + Sancho-Rubio + sweep kernels (n = 17: forward + way-back kernel when the launch holds real-axis
+  // CTAs) + one combine per launch that holds contour CTAs + 2-level reduce
+  int sweeps = 0, combines = 0;
+  for (long long b = 0; b < bp->total_cta; b += bp->slots) {
+    sweeps += (bp->n == 17 && b + bp->slots > bp->n_eq_cta) ? 2 : 1;
+    if (b < bp->n_eq_cta) ++combines;
+  }
+  out->kernel_launches = 1 + 1 + sweeps + combines + 2;
 }
 
 }  // namespace negf

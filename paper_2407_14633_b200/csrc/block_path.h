@@ -29,7 +29,6 @@ negf_status block_path_check(BlockPath* bp);
 negf_status block_path_copy_sigma(BlockPath* bp, double2* sigma_dev, cudaStream_t s);
 void block_path_plan(BlockPath* bp, negf_plan_info* out);
 void block_path_destroy(BlockPath* bp);
-void block_path_set_pivot_threshold(double theta);   // process-wide; <= 0 restores the default
 
 namespace blk {
 
@@ -60,6 +59,7 @@ struct SrLaunch {
   int maxit;
   int* max_iters;             // device scalar, atomicMax
   int* noconv_flag;           // device scalar
+  unsigned long long* iters_total;   // device scalar: decimation passes summed over all tasks
 };
 cudaError_t launch_sancho_rubio(int nb, const SrLaunch& p, cudaStream_t s);
 
@@ -69,6 +69,7 @@ cudaError_t launch_sancho_rubio(int nb, const SrLaunch& p, cudaStream_t s);
 struct SweepLaunch {
   int C, N, K_eq, K_neq;
   int geq, gneq;              // energy groups per channel: ceil(K / TPC)
+  long long n_eq_cta;         // number of contour CTAs = C * geq * 2 (they come first in the global numbering)
   long long cta_begin;
   int n_cta;
   const double* U;

@@ -136,7 +136,8 @@ void hook_begin(void* ctx, int kind) {
   negf_handle* h = static_cast<negf_handle*>(ctx);
   if (!h->profile) return;
   ProfEntry ent;
-  ent.kind = kind == 0 ? K_SANCHO : (kind == 1 ? K_BLOCK_SWEEP : (kind == 3 ? K_BLOCK_COMBINE : K_REDUCE));
+  static const int map[4] = {K_SANCHO, K_BLOCK_SWEEP, K_REDUCE, K_BLOCK_COMBINE};
+  ent.kind = (kind >= 0 && kind < 4) ? map[kind] : K_MISC;
   ent.a = prof_event(h);
   ent.b = prof_event(h);
   cudaEventRecord(ent.a, h->stream);
@@ -236,10 +237,6 @@ negf_status run_sweeps(negf_handle* h) {
 }  // namespace
 
 extern "C" const char* negf_last_error(void) { return negf::g_err; }
-extern "C" negf_status negf_set_pivot_threshold(double theta) {
-  negf::block_path_set_pivot_threshold(theta);
-  return NEGF_OK;
-}
 extern "C" const char* negf_version(void) { return "negf_b200 0.1 (sm_100a)"; }
 
 extern "C" negf_status negf_destroy(negf_handle* h) {

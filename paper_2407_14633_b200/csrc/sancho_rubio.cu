@@ -205,6 +205,7 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
   }
   if (active && r == 0) {
     atomicMax(p.max_iters, iters);
+    atomicAdd(p.iters_total, (unsigned long long)iters);
     if (!frozen) atomicExch(p.noconv_flag, 1);
   }
 

@@ -84,20 +84,16 @@ def test_random_complex_blocks_vs_dense_definition(n, sparse):
 
 
 def test_forced_column_search_matches():
-    """theta = 1e150 rejects every diagonal candidate, so every elimination step takes the
-    partial-pivoting search path; the results must still match the dense definition."""
-    from paper_2407_14633_b200 import negf_set_pivot_threshold
+    """negf_config.pivot_theta = 1e150 rejects every diagonal candidate, so every elimination step
+    takes the partial-pivoting search path; the results must still match the dense definition."""
     wl3 = wlmod.make_config(3, N=10, K_neq=20, K_eq=5)
     wlr = _random_block_workload(5, N=11, K_neq=17, K_eq=4, seed=77)
-    refs = [od.charge_and_transmission(w) for w in (wl3, wlr)]
-    try:
-        negf_set_pivot_threshold(1e150)
-        for w, (n_ref, T_ref) in zip((wl3, wlr), refs):
-            n, T = _gpu_run(w)
-            assert_parity(n, n_ref, f"{w.name} forced-search charge")
-            assert_parity(T, T_ref, f"{w.name} forced-search T(E)")
-    finally:
-        negf_set_pivot_threshold(0.0)
+    wl17 = _random_block_workload(17, N=7, K_neq=11, K_eq=3, seed=78, sparse=True)
+    for w in (wl3, wlr, wl17):
+        n_ref, T_ref = od.charge_and_transmission(w)
+        n, T = _gpu_run(w, pivot_theta=1e150)
+        assert_parity(n, n_ref, f"{w.name} forced-search charge")
+        assert_parity(T, T_ref, f"{w.name} forced-search T(E)")
 
 
 def test_config4_shrunk_multi_channel():

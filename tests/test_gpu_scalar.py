@@ -138,3 +138,88 @@ def test_landauer_reductions():
     assert abs(cond.item() - 4.0) < 1e-4             # 4 open subbands at E = 0.6 eV
     assert abs(cur.item()) < 1e-12                   # mu_s == mu_d
     h.negf_destroy()
+
+
+@pytest.mark.parametrize("cfg,kw", [(2, dict(N=18, K_neq=21, K_eq=0)), (1, dict(N=30, K_neq=40)),
+                                    (3, dict(N=9, K_neq=10, K_eq=0)), (4, dict(C=3, N=8, K_neq=9, K_eq=0))])
+def test_current_and_conductance_vs_definition(cfg, kw):
+    """negf_current against the oracle's currents by the definition of eq.(5)
+    (Tr[F_l Gamma_l A + i Gamma_l G^<] from the dense Green's function) and the
+    conductance of eq.(6), at mu_S != mu_D, scalar and block handles, several channels."""
+    import torch
+    from paper_2407_14633_b200 import Negf
+    wl = wlmod.make_config(cfg, **kw)
+    assert wl.mu_s != wl.mu_d
+    I_ref, I_D, G_ref = od.landauer_dense(wl)
+    assert np.all(np.abs(I_ref + I_D) < 1e-9 * np.abs(I_ref))          # conservation (P6) in the oracle
+    h = Negf.from_workload(wl)
+    h.negf_set_potential(torch.tensor(wl.phi, dtype=torch.float64, device="cuda"))
+    cur = torch.empty(wl.C, dtype=torch.float64, device="cuda")
+    cond = torch.empty(wl.C, dtype=torch.float64, device="cuda")
+    h.negf_current(cur, cond)
+    h.negf_sync()
+    assert_parity(cur.cpu().numpy(), I_ref, f"config{cfg} current")
+    assert_parity(cond.cpu().numpy(), G_ref, f"config{cfg} conductance")
+    h.negf_destroy()
+
+
+def test_current_of_ideal_tube_on_gpu():
+    """Pin on the CUDA path alone: I = (g_s e/h) M (mu_S - mu_D) with M = 2 open modes (library units:
+    eV), both chemical potentials inside the first plateau of the ideal (17,0) tube."""
+    import torch
+    from paper_2407_14633_b200 import Negf
+    mu_s, mu_d, kT = 0.42, 0.36, 0.004
+    wl = wlmod.make_config(2, N=16, K_neq=160, K_eq=0)
+    wl.phi[:] = 0.0
+    wl.mu_s, wl.mu_d, wl.kT = mu_s, mu_d, kT
+    wl.z_neq, wl.w_neq = wlmod.real_axis_gauss_legendre(mu_d - 14 * kT, mu_s + 14 * kT, 160, eta=1e-9)
+    h = Negf.from_workload(wl)
+    h.negf_set_potential(torch.tensor(wl.phi, dtype=torch.float64, device="cuda"))
+    cur = torch.empty(1, dtype=torch.float64, device="cuda")
+    h.negf_current(cur, None)
+    h.negf_sync()
+    assert abs(cur.item() - 2.0 * (mu_s - mu_d)) < 1e-6
+    h.negf_destroy()
+
+
+@pytest.mark.parametrize("cfg,kw", [(2, dict(N=21, K_neq=8, K_eq=8)), (3, dict(N=10, K_neq=8, K_eq=8)),
+                                    (4, dict(C=2, N=9, K_neq=8, K_eq=8))])
+def test_equilibrium_only_and_neutral_contours_vs_definition(cfg, kw):
+    """the equilibrium-only contour (two arcs + the enclosed Fermi poles
+    z_p = mu + i pi kT (2p+1) as extra (z, W) points, no real-axis points) and the neutral-charge
+    contour run through the same kernels; charge per ring against the dense definition."""
+    base = wlmod.make_config(cfg, **kw)
+    for wl in (wlmod.equilibrium_variant(base, mu=-0.03, K_eq=24), wlmod.neutral_variant(base, K_eq=24)):
+        assert wl.K_neq == 0
+        n_ref, _ = od.charge_and_transmission(wl)
+        import torch
+        from paper_2407_14633_b200 import Negf
+        h = Negf.from_workload(wl)
+        n = torch.empty((wl.C, wl.N), dtype=torch.float64, device="cuda")
+        h.negf_set_potential(torch.tensor(wl.phi, dtype=torch.float64, device="cuda"))
+        h.negf_charge(n)
+        h.negf_sync()
+        assert_parity(n.cpu().numpy(), n_ref, f"{wl.name} charge")
+        h.negf_destroy()
+
+
+def test_equilibrium_only_equals_two_part_on_gpu():
+    """The 8(f)-3 pin on the CUDA path alone: equilibrium-only contour == two-part path at mu_S = mu_D
+    (to the 2 eta G G^dagger term, ~1e-7) on a chain whose band edges are far from the Fermi window."""
+    import torch
+    from paper_2407_14633_b200 import Negf
+    base = wlmod.make_config(1, N=40, K_neq=8)
+    mu, e_b = 0.3, -6.0
+    weq = wlmod.equilibrium_variant(base, mu=mu, K_eq=48, e_b=e_b)
+    w2 = wlmod.two_part_equilibrium_variant(base, mu=mu, K_eq=48, K_neq=160)
+    w2.z_eq, w2.w_eq = wlmod.contour_semicircle(e_b, mu - wlmod.F_TAIL * base.kT, 48, mu, base.kT)
+    out = []
+    for wl in (weq, w2):
+        h = Negf.from_workload(wl)
+        n = torch.empty((wl.C, wl.N), dtype=torch.float64, device="cuda")
+        h.negf_set_potential(torch.tensor(wl.phi, dtype=torch.float64, device="cuda"))
+        h.negf_charge(n)
+        h.negf_sync()
+        out.append(n.cpu().numpy())
+        h.negf_destroy()
+    assert np.max(np.abs(out[0] - out[1]) / out[1]) < 2e-6

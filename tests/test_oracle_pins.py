@@ -291,6 +291,51 @@ def test_p5_spectral_identity_and_hermiticity(cfg):
         assert abs(TLR - TRL) < 1e-12 * max(1.0, abs(TLR))
 
 
+# ------------------------------------------------------------------ eq.(5)-(6): current, conductance
+
+def _ideal_tube(kind, N, E_lo, E_hi, K, mu_s, mu_d, kT, eta=1e-9):
+    w = wlmod.make_config(3 if kind == "block" else 2, N=N, K_neq=K, K_eq=0)
+    w.phi[:] = 0.0
+    w.z_neq, w.w_neq = wlmod.real_axis_gauss_legendre(E_lo, E_hi, K, eta)
+    w.mu_s, w.mu_d, w.kT = mu_s, mu_d, kT
+    return w
+
+
+@pytest.mark.parametrize("kind", ["scalar", "block"])
+def test_f1_landauer_current_of_ideal_tube_counts_open_modes(kind):
+    """eq.(5): for an ideal tube every open subband transmits perfectly, so at low kT
+    with both chemical potentials inside one transmission plateau I = (g_s e/h) M (mu_S - mu_D),
+    M = number of open modes (2 between the first subband edge 0.2713 eV and the second 0.5127 eV);
+    I_S + I_D = 0 (current conservation, P6); G = M G_0 (eq.(6))."""
+    mu_s, mu_d, kT = 0.42, 0.36, 0.004
+    lo, hi = mu_d - 14 * kT, mu_s + 14 * kT                   # [0.304, 0.476] inside the plateau
+    w = _ideal_tube(kind, 6, lo, hi, 160, mu_s, mu_d, kT)
+    I_S, I_D, G = od.landauer_dense(w)
+    assert abs(I_S[0] - 2.0 * (mu_s - mu_d)) < 1e-6           # O(N eta) + Fermi tails exp(-14)
+    assert abs(I_S[0] + I_D[0]) < 1e-9 * abs(I_S[0])
+    assert abs(G[0] - 2.0) < 1e-5
+
+
+def test_f1_current_equals_transmission_form_and_changes_sign():
+    """Tr[F_S Gamma_S A + i Gamma_S G^<] = T_SD (F_S - F_D) for two leads (algebra on eq.(5)); the
+    definition-based oracle must agree with the T(E)-based sum of the other oracle path, vanish at
+    mu_S = mu_D and flip sign with the bias."""
+    w = wlmod.make_config(2, N=14, K_neq=12, K_eq=0)
+    I_S, I_D, _ = od.landauer_dense(w)
+    _, T = od.charge_and_transmission(w)
+    fS = od.fermi_real(w.z_neq.real, w.mu_s, w.kT)
+    fD = od.fermi_real(w.z_neq.real, w.mu_d, w.kT)
+    expect = np.sum(w.w_neq * T[0] * (fS - fD))
+    assert abs(I_S[0] - expect) < 1e-12 * abs(expect)
+    assert abs(I_S[0] + I_D[0]) < 1e-10 * abs(I_S[0])         # real H: T_SD = T_DS exactly (P6)
+    w.mu_s, w.mu_d = w.mu_d, w.mu_s
+    I_S2, _, _ = od.landauer_dense(w)
+    assert abs(I_S2[0] + I_S[0]) < 1e-12 * abs(I_S[0])
+    w.mu_d = w.mu_s
+    I_S3, _, _ = od.landauer_dense(w)
+    assert abs(I_S3[0]) < 1e-14
+
+
 # ------------------------------------------------------------------ P7: real space == sum of modes
 
 def test_p7_real_space_equals_sum_of_modes():
@@ -339,6 +384,94 @@ def test_p9_biased_uniform_chain_density():
     w = _chain_workload(N=14, K_neq=128, K_eq=48, mu_s=mu_s, mu_d=mu_d)
     n, _ = od.charge_and_transmission(w)
     assert np.max(np.abs(n[0] / w.deg - val)) < 5e-7
+
+
+# ------------------------------------------------------------------ contours and grids
+
+def test_f3_equilibrium_contour_closed_form():
+    """contour_equilibrium on a function with a closed-form answer: for G(z) = 1/(z - a), a in the
+    lower half plane, int_{e_b}^{E_u} G F dE is a plain 1D integral (scipy.quad); the contour sum
+    (two arcs + enclosed Fermi poles with weight -2 pi i kT) must reproduce it.  A wrong pole sign,
+    weight or count misses by ~2 pi kT |G| ~ 0.1."""
+    kT, mu, eb = 0.0259, -0.05, -8.5
+    G = lambda z: 1.0 / (z + 1.0 + 0.3j) + 0.5 / (z - 0.02 + 0.05j)
+    z, W, m = wlmod.contour_equilibrium(eb, mu, kT, 64)
+    assert m == 3 and len(z) == 64 + 64 + 3
+    e_u = mu + 2 * np.pi * kT * m
+    assert e_u >= mu + wlmod.F_TAIL * kT
+    f = lambda E: 1.0 / (1.0 + np.exp((E - mu) / kT))
+    re = integrate.quad(lambda E: (G(E) * f(E)).real, eb, e_u, limit=2000, points=[mu, -1, 0.02])[0]
+    im = integrate.quad(lambda E: (G(E) * f(E)).imag, eb, e_u, limit=2000, points=[mu, -1, 0.02])[0]
+    assert abs(np.sum(W * G(z)) - (re + 1j * im)) < 5e-6
+
+
+@pytest.mark.parametrize("which", ["chain", "tube"])
+def test_f3_equilibrium_only_equals_two_part_result(which):
+    """PAPER.md:96: at equilibrium (mu_S = mu_D) the residue-theorem contour alone gives the charge;
+    it must equal the two-part result of eq.(4) at mu_S = mu_D (SURVEY 8(f)-3 pin).  Devices whose
+    van Hove edges lie outside the Fermi window, so that the two-part real-axis quadrature is itself
+    accurate; the remaining difference is the 2 eta G G^dagger term of P5 (~1e-7)."""
+    if which == "chain":
+        base = wlmod.make_config(1, N=12, K_neq=8)
+        mu, e_b = 0.3, -6.0
+    else:
+        base = wlmod.make_config(3, N=8, K_neq=8, K_eq=8)
+        base.phi[:] = 0.01 * np.linspace(-1.0, 1.0, 8)
+        base.kT = 0.004
+        mu, e_b = 0.4, wlmod.E_B                           # window [0.34, 0.46] inside the first plateau
+    weq = wlmod.equilibrium_variant(base, mu=mu, K_eq=48, e_b=e_b)
+    n_eq, _ = od.charge_and_transmission(weq)
+    w2 = wlmod.two_part_equilibrium_variant(base, mu=mu, K_eq=48, K_neq=128)
+    w2.z_eq, w2.w_eq = wlmod.contour_semicircle(e_b, mu - wlmod.F_TAIL * base.kT, 48, mu, base.kT)
+    n_2, _ = od.charge_and_transmission(w2)
+    assert weq.K_neq == 0 and weq.extra["n_poles"] == 3
+    assert np.max(np.abs(n_eq - n_2) / n_2) < 2e-6
+
+
+def test_f3_neutral_charge_of_ideal_tube_is_half_filling():
+    """rho_0 ("E_l = E_u = 0"): all states below the charge-neutrality point filled.
+    For the ideal tube (bipartite lattice, phi = 0) that is exactly one electron per atom:
+    n = deg * 17 / 2 = 17 per ring."""
+    w = wlmod.neutral_variant(wlmod.make_config(3, N=6, K_neq=4, K_eq=4), K_eq=48)
+    w.phi[:] = 0.0
+    n, _ = od.charge_and_transmission(w)
+    assert np.max(np.abs(n - 17.0)) < 1e-6
+    ws = wlmod.neutral_variant(wlmod.make_config(2, N=9, K_neq=4, K_eq=4), K_eq=48)
+    ws.phi[:] = 0.0
+    n, _ = od.charge_and_transmission(ws)
+    assert np.max(np.abs(n - 17.0)) < 1e-6
+
+
+def test_f2_three_segment_grid():
+    """PAPER.md:353: three sub-regions with their own density of points per kT, Gauss-Legendre in each;
+    the paper's densities (500, 1600, 50) on its window give ~12 000 points."""
+    kT = 0.0259
+    e_min, e_max = -0.1 - 14 * kT, 0.0 + 14 * kT
+    z, w, counts = wlmod.real_axis_three_segment(e_min, -0.30, -0.25, e_max, kT, (500, 1600, 50))
+    assert len(z) == sum(counts) == len(w)
+    assert counts == (int(np.ceil(500 * (-0.30 - e_min) / kT)), int(np.ceil(1600 * 0.05 / kT)),
+                      int(np.ceil(50 * (e_max + 0.25) / kT)))
+    assert 5000 < len(z) < 20000
+    E = z.real
+    assert np.all(np.diff(E) > 0) and np.all(z.imag == wlmod.ETA)
+    assert abs(w.sum() - (e_max - e_min)) < 1e-13                     # weights cover the window exactly
+    assert abs(np.sum(w * E ** 5) - (e_max ** 6 - e_min ** 6) / 6) < 1e-13   # exact for polynomials
+    # a sharp peak inside the dense segment is integrated to 1e-9; with one 64-point rule it is not
+    lor = lambda x: (1e-3 / np.pi) / ((x + 0.27) ** 2 + 1e-6)
+    exact = (np.arctan((e_max + 0.27) / 1e-3) - np.arctan((e_min + 0.27) / 1e-3)) / np.pi
+    assert abs(np.sum(w * lor(E)) - exact) < 1e-9
+    z1, w1 = wlmod.real_axis_gauss_legendre(e_min, e_max, 64)
+    assert abs(np.sum(w1 * lor(z1.real)) - exact) > 1e-2
+    # degenerate limits collapse to fewer segments
+    z2, w2, c2 = wlmod.real_axis_three_segment(e_min, e_min - 1.0, e_min - 0.5, e_max, kT, (500, 1600, 50))
+    assert c2[0] == 0 and c2[1] == 0 and abs(w2.sum() - (e_max - e_min)) < 1e-13
+
+
+def test_f2_refine_segment_limits_brackets_the_peak():
+    E = np.linspace(-0.4, 0.3, 701)
+    integrand = 1.0 / np.sqrt(np.abs(E + 0.2713) + 1e-4)              # van Hove-like edge
+    e_s, l1, l2 = wlmod.refine_segment_limits(E, integrand, 0.0259)
+    assert abs(e_s + 0.2713) < 1e-3 and l1 == e_s - 3 * 0.0259 and l2 == e_s + 0.0259
 
 
 # ------------------------------------------------------------------ P10: brute force, O1 vs O3

@@ -21,6 +21,13 @@ from .configs import (  # noqa: F401
     cnt_realspace_couplings,
     barrier_profile,
     contour_semicircle,
+    contour_equilibrium,
+    contour_neutral,
+    real_axis_three_segment,
+    refine_segment_limits,
+    equilibrium_variant,
+    two_part_equilibrium_variant,
+    neutral_variant,
     real_axis_gauss_legendre,
     real_axis_uniform,
     fermi,

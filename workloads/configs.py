@@ -149,6 +149,78 @@ def contour_semicircle(e_b: float, e_min: float, K: int, mu_min: float, kT: floa
     return z.astype(np.complex128), W.astype(np.complex128)
 
 
+def contour_equilibrium(e_b: float, mu: float, kT: float, K: int, f_tail: float = F_TAIL, K_cap: int = 64):
+    """Equilibrium-only contour ("At equilibrium ... the charge density
+    can be calculated solely using the residue theorem by setting E_l = E_u = mu + f k_bT").
+
+    The real-axis integral int_{e_b}^{E_u} G^R F dE is closed in the upper half plane, where G^R is
+    analytic and the Fermi function has the simple poles z_p = mu + i pi kT (2p + 1) with residue -kT:
+        int_{e_b}^{E_u} G F dE = -int_arcs G F dz - 2 pi i kT sum_{p inside} G(z_p).
+    The path is two semicircles: the large one of ``contour_semicircle`` from e_b to mu - r (left of
+    the Fermi edge, where F is smooth) and a small cap of radius r around mu from mu - r to
+    E_u = mu + r, r = 2 pi kT m with the smallest integer m for which r >= f_tail kT -- the cap
+    crosses Re z = mu midway between the poles m - 1 and m, so that no pole sits on the path and
+    the K_cap Gauss-Legendre points of the cap resolve the pole structure (a single large semicircle
+    crossing the pole line converges only at ~500 points).  Node list: K points of the large arc,
+    K_cap points of the cap, then the m enclosed poles with weight W_p = -2 pi i kT.
+    Returns (z, W, number of poles).  DESIGN.md reading R24."""
+    m = int(np.ceil(f_tail / (2.0 * np.pi)))
+    r = 2.0 * np.pi * kT * m
+    za, Wa = contour_semicircle(e_b, mu - r, K, mu, kT)
+    zc, Wc = contour_semicircle(mu - r, mu + r, K_cap, mu, kT)
+    zp = mu + 1j * np.pi * kT * (2.0 * np.arange(m) + 1.0)          # Im z_p < r
+    Wp = np.full(m, -2.0j * np.pi * kT, dtype=np.complex128)
+    return (np.concatenate([za, zc, zp]).astype(np.complex128),
+            np.concatenate([Wa, Wc, Wp]).astype(np.complex128), m)
+
+
+def contour_neutral(e_b: float, K: int, e_u: float = 0.0):
+    """Contour of the neutral charge density rho_0 ("computed with E_l = E_u = 0"):
+    all states below E = 0 -- the charge-neutrality point of the tube -- filled, no thermal smearing,
+    so the occupation factor is 1 on the whole arc and no pole is enclosed (reading R24)."""
+    if K == 0:
+        return np.zeros(0, np.complex128), np.zeros(0, np.complex128)
+    x, w = np.polynomial.legendre.leggauss(K)
+    theta = 0.5 * np.pi * (x + 1.0)
+    c = 0.5 * (e_b + e_u)
+    R = 0.5 * (e_u - e_b)
+    z = c + R * np.exp(1j * theta)
+    W = -1j * R * np.exp(1j * theta) * (0.5 * np.pi * w)
+    return z.astype(np.complex128), W.astype(np.complex128)
+
+
+def real_axis_three_segment(e_min: float, e_l1: float, e_l2: float, e_max: float, kT: float,
+                            density=(500.0, 1600.0, 50.0), eta: float = ETA, k_max: int = 1 << 20):
+    """Semi-adaptive real-axis path of PAPER.md:353: [e_min, e_l1], [e_l1, e_l2],
+    [e_l2, e_max], each with its own density of integration points per kT (the paper's largest
+    device: (500, 1600, 50), ~12 000 points in total) and its own Gauss-Legendre rule.  Empty
+    segments (e.g. e_l1 <= e_min) are dropped.  Returns (z = E + i eta, w, points per segment)."""
+    edges = [e_min, min(max(e_l1, e_min), e_max), min(max(e_l2, e_l1, e_min), e_max), e_max]
+    zs, ws, counts = [], [], []
+    for s in range(3):
+        lo, hi = edges[s], edges[s + 1]
+        if hi - lo <= 0.0:
+            counts.append(0)
+            continue
+        k = int(min(max(np.ceil(density[s] * (hi - lo) / kT), 2), k_max))
+        z, w = real_axis_gauss_legendre(lo, hi, k, eta)
+        zs.append(z)
+        ws.append(w)
+        counts.append(k)
+    return np.concatenate(zs), np.concatenate(ws), tuple(counts)
+
+
+def refine_segment_limits(E, integrand, kT: float, a: float = 3.0, b: float = 1.0):
+    """The refresh step of the semi-adaptive path: locate the peak E_s of the integrand
+    A_1 F_1 + A_2 F_2 at the centre of the channel and put the dense segment around it,
+    E_l1 = E_s - a kT, E_l2 = E_s + b kT (a = 3, b = 1 "typically").  The paper prints
+    "E_l1 = E_l1 - akT", read as E_s - akT (reading R25).  Returns (E_s, E_l1, E_l2)."""
+    E = np.asarray(E, dtype=np.float64)
+    k = int(np.argmax(np.asarray(integrand, dtype=np.float64)))
+    e_s = float(E[k])
+    return e_s, e_s - a * kT, e_s + b * kT
+
+
 def _window(mu_s: float, mu_d: float, kT: float):
     return min(mu_s, mu_d) - F_TAIL * kT, max(mu_s, mu_d) + F_TAIL * kT
 
@@ -327,3 +399,30 @@ def make_config(idx: int, **overrides) -> Workload:
     """``make_config(3, N=40, K_neq=16, K_eq=8)`` gives the shrunk variant of
     config 3 produced by the same generator."""
     return _FACTORIES[idx](**overrides)
+
+
+def equilibrium_variant(wl: Workload, mu: Optional[float] = None, K_eq: int = 64, e_b: float = E_B) -> Workload:
+    """Equilibrium-only evaluation of a workload: mu_S = mu_D = mu, no real-axis points,
+    the contour of ``contour_equilibrium`` with the enclosed Fermi poles appended."""
+    mu = wl.mu_s if mu is None else mu
+    z, W, n_poles = contour_equilibrium(e_b, mu, wl.kT, K_eq)
+    return replace(wl, name=wl.name + "_equilibrium", mu_s=mu, mu_d=mu, z_eq=z, w_eq=W,
+                   z_neq=np.zeros(0, np.complex128), w_neq=np.zeros(0, np.float64),
+                   extra=dict(wl.extra, n_poles=n_poles))
+
+
+def two_part_equilibrium_variant(wl: Workload, mu: Optional[float] = None, K_eq: int = 64,
+                                 K_neq: int = 256) -> Workload:
+    """The same physical quantity through the two-part path of eq.(4) at mu_S = mu_D = mu (the pin of the
+    equilibrium-only contour: both must give the same charge)."""
+    mu = wl.mu_s if mu is None else mu
+    z_eq, w_eq, z_neq, w_neq = _grids(K_neq, K_eq, mu_s=mu, mu_d=mu, kT=wl.kT, eta=wl.eta)
+    return replace(wl, name=wl.name + "_twopart", mu_s=mu, mu_d=mu, z_eq=z_eq, w_eq=w_eq,
+                   z_neq=z_neq, w_neq=w_neq)
+
+
+def neutral_variant(wl: Workload, K_eq: int = 64, e_b: float = E_B) -> Workload:
+    """Neutral charge density rho_0 of a workload: ``contour_neutral``, no real-axis points."""
+    z, W = contour_neutral(e_b, K_eq)
+    return replace(wl, name=wl.name + "_neutral", z_eq=z, w_eq=W,
+                   z_neq=np.zeros(0, np.complex128), w_neq=np.zeros(0, np.float64))
