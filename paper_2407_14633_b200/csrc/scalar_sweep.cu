@@ -15,6 +15,8 @@
 // as single tasks (right-connected pass stored as complex, left-connected pass on the fly).
 // Energy reduction (eq.(4)): each warp transposes 16 rings x 32 energies through shared
 // memory, sums them and writes one partial per ring; a deterministic second stage sums the warps.
+#include <algorithm>
+
 #include "negf_internal.h"
 
 namespace negf {
@@ -358,11 +360,11 @@ scalar_contour_kernel(const ScalarLaunch p, const int n_warps) {
 // of eq.(4): -(deg/pi) Im[W_k G_(i,i)], summed over the 32 (mode, energy) tasks of a warp pair.
 // grid = (ring chunks of 32 * kWarpsPerBlock... see launcher, pairs); one warp per (pair, 32 rings).
 __global__ void __launch_bounds__(128)
-scalar_combine_kernel(const ScalarLaunch p, const int n_pairs) {
+scalar_combine_kernel(const ScalarLaunch p, const int pair0) {
   __shared__ double tiles[4][32][33];
   const int lane = threadIdx.x & 31;
   const int wib = threadIdx.x >> 5;
-  const int pair = blockIdx.y;
+  const int pair = pair0 + blockIdx.y;
   const int N = p.N;
   const int i0 = (blockIdx.x * 4 + wib) * 32;
   if (i0 >= N) return;
@@ -429,9 +431,11 @@ cudaError_t launch_scalar_sweep(const ScalarLaunch& p, cudaStream_t s) {
     if ((e = cudaStreamWaitEvent(p.side, p.ev_fork, 0)) != cudaSuccess) return e;
     scalar_contour_kernel<<<(n_c + kWarpsPerBlock - 1) / kWarpsPerBlock, kWarpsPerBlock * 32, 0, p.side>>>(p, n_c);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    dim3 grid((p.N + 127) / 128, n_c / 2);
-    scalar_combine_kernel<<<grid, 128, 0, p.side>>>(p, n_c / 2);
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    for (int pair0 = 0; pair0 < n_c / 2; pair0 += 65535) {   // grid.y is limited to 65535
+      dim3 grid((p.N + 127) / 128, std::min(65535, n_c / 2 - pair0));
+      scalar_combine_kernel<<<grid, 128, 0, p.side>>>(p, pair0);
+      if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    }
     if ((e = cudaEventRecord(p.ev_join, p.side)) != cudaSuccess) return e;
   }
   if (n_r > 0) {

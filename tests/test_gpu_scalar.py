@@ -223,3 +223,38 @@ def test_equilibrium_only_equals_two_part_on_gpu():
         out.append(n.cpu().numpy())
         h.negf_destroy()
     assert np.max(np.abs(out[0] - out[1]) / out[1]) < 2e-6
+
+
+def test_table2_long_channel_workload():
+    """SURVEY 8(f)-4 workload (Table 2): N = 524 288 rings, 90 contour points
+    (equilibrium contour with the Fermi poles), 8 doubly-degenerate modes.  Shrunk (N = 300) against the
+    dense definition in full; at FULL length in the launch configuration bench.py times, the charge of
+    sampled (mode, contour point) subsets against the C++ tier O3 oracle, every ring."""
+    import torch
+    from paper_2407_14633_b200 import Negf
+    from oracle import negf_rgf_omp as omp
+
+    def gpu_charge(wl):
+        h = Negf.from_workload(wl)
+        n = torch.empty((wl.C, wl.N), dtype=torch.float64, device="cuda")
+        h.negf_set_potential(torch.tensor(wl.phi, dtype=torch.float64, device="cuda"))
+        h.negf_charge(n)
+        h.negf_sync()
+        h.negf_destroy()
+        return n.cpu().numpy()
+
+    small = wlmod.table2(N=300)
+    assert small.K_eq == 90 and small.K_neq == 0 and small.n_modes == 8
+    n_ref, _ = od.charge_and_transmission(small)
+    assert_parity(gpu_charge(small), n_ref, "table2 shrunk charge")
+    full = wlmod.table2()
+    assert full.N == 524288
+    n_full = gpu_charge(full)                      # the full launch configuration: all 720 chains
+    assert np.all(np.isfinite(n_full)) and np.all(n_full > 0)
+    # linear in the contour points: the sampled subsets are themselves valid workloads
+    sub = full.subset(eq_idx=[0, 11, 22, 23, 55, 86, 87, 89])
+    sub.coup_even, sub.coup_odd, sub.mode_weight, sub.n_modes = (full.coup_even[[0, 7]], full.coup_odd[[0, 7]],
+                                                                 full.mode_weight[[0, 7]], 2)
+    n_sub = gpu_charge(sub)
+    n_ref, _ = omp.charge_and_transmission(sub)
+    assert_parity(n_sub, n_ref, "table2 full-length charge of sampled chains, every ring")

@@ -15,6 +15,7 @@ from .configs import (  # noqa: F401
     config3,
     config4,
     config5,
+    table2,
     make_config,
     scalar_twin,
     cnt_mode_couplings,

@@ -392,7 +392,30 @@ def scalar_twin(block_wl: Workload) -> Workload:
                    mode_weight=np.ones(CNT_N), lead_kind=0)
 
 
-_FACTORIES = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
+def table2(N: int = 524288, n_modes: int = 8, K_arc: int = 23, K_cap: int = 64, seed: int = 2002,
+           mu: float = 0.0) -> Workload:
+    """The long-channel, few-energy workload of the paper's Table 2:
+    N = 524 288 rings, equilibrium (contour only), 90 contour points, modes 1..n_modes of the (17,0)
+    tube in mode space, each doubly degenerate ("modes 1 to 8 (all doubly-degenerate)").
+    90 points = 23 on the large arc + 64 on the cap around mu + the 3 enclosed Fermi poles
+    (``contour_equilibrium``).  Potential: the gate barrier of configs 2-5 stretched to N rings, height
+    0.3 eV, +-5 meV noise.  The parallelism over energies is scarce here (90 x 8 chains): the sweep is a
+    serial pass over 524 288 rings per chain."""
+    rng = np.random.default_rng(seed)
+    U = _gate_potential(N, 0.3, 0.005, rng)
+    j = np.arange(1, n_modes + 1, dtype=np.float64)
+    even = (2.0 * T_HOP * np.cos(np.pi * j / CNT_N)).astype(np.complex128)
+    odd = np.full(n_modes, T_HOP, dtype=np.complex128)
+    z, W, n_poles = contour_equilibrium(E_B, mu, KT, K_arc, K_cap=K_cap)
+    return Workload(
+        name="table2", kind="scalar", C=1, N=N, n=1, n_modes=n_modes,
+        coup_even=even, coup_odd=odd, mode_weight=np.full(n_modes, 2.0),
+        phi=(-U)[None, :].copy(), z_eq=z, w_eq=W,
+        z_neq=np.zeros(0, np.complex128), w_neq=np.zeros(0, np.float64),
+        mu_s=mu, mu_d=mu, lead_kind=0, seed=seed, extra={"n_poles": n_poles})
+
+
+_FACTORIES = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5, 6: table2}
 
 
 def make_config(idx: int, **overrides) -> Workload:
