@@ -131,6 +131,19 @@ NEGF_API negf_status negf_self_energy(negf_handle* h, negf_c64* sigma_dev);
  * Either output may be NULL. */
 NEGF_API negf_status negf_current(negf_handle* h, double* current_dev, double* conductance_dev);
 
+/* Semi-adaptive real-axis path, the device side ("compute the integrand at
+ * the center of the channel as a function of energy, obtain the peak of the singularity E_s").
+ * negf_set_probe selects the ring (0 <= ring < N; ring < 0 switches the probe off) whose per-energy
+ * contributions the sweep kernels record from then on; it invalidates cached results.
+ * negf_integrand_peak runs the sweep if needed and writes, per channel c,
+ *   integrand[c][k] = sum_modes mode_weight (F_S Tr_ring A_S,(r,r) + F_D Tr_ring A_D,(r,r))(E_k)   [C][K_neq]
+ * (the integrand of the second term of eq.(4) without 1/2pi, deg and the quadrature weight), the index
+ * k_peak[c] of its first maximum and E_peak[c] = Re z_neq[k_peak[c]].  Any of the three outputs may be NULL.
+ * NEGF_ESTATE without a probe ring or a potential; NEGF_EINVAL for a handle without real-axis points. */
+NEGF_API negf_status negf_set_probe(negf_handle* h, int32_t ring);
+NEGF_API negf_status negf_integrand_peak(negf_handle* h, double* integrand_dev, int32_t* k_peak_dev,
+                                         double* E_peak_dev);
+
 /* Host-buffer convenience path (the end-to-end call): copies phi from HOST memory, runs
  * negf_set_potential + negf_charge (+ transmission), copies n (and T if T_host != NULL) back to HOST
  * memory and synchronises the stream. */

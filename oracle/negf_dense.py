@@ -193,3 +193,32 @@ def landauer_dense(wl, channels=None):
                 I_D[c] += wgt * wl.w_neq[k] * iD
                 G[c] += wgt * wl.w_neq[k] * T * dfdE[k]
     return I_S, I_D, G
+
+
+def integrand_dense(wl, ring: int, channels=None):
+    """The integrand of the second term of eq.(4) at one ring as a function of energy (PAPER.md:353,
+    "the integrand A_1 F_1 + A_2 F_2 at the center of the channel"), by the definition:
+      I_c(E_k) = sum_modes mode_weight (F_S Tr_ring A_S,(r,r) + F_D Tr_ring A_D,(r,r))(E_k),
+    A_l = G^R Gamma_l G^R^dagger from the dense inverse.  Returns I[C, K_neq]."""
+    chans = range(wl.C) if channels is None else channels
+    out = np.zeros((wl.C, wl.K_neq))
+    fS = fermi_real(wl.z_neq.real, wl.mu_s, wl.kT)
+    fD = fermi_real(wl.z_neq.real, wl.mu_d, wl.kT)
+    for c in chans:
+        U = -wl.phi[c]
+        units = ([(wl.coup_even[j:j + 1], wl.coup_odd[j:j + 1], 1, 0, wl.mode_weight[j])
+                  for j in range(wl.n_modes)] if wl.kind == "scalar"
+                 else [(wl.coup_even, wl.coup_odd, wl.n, 1, 1.0)])
+        for ce, co, n, lead_kind, wgt in units:
+            D = U.shape[0] * n
+            rows = slice(ring * n, (ring + 1) * n)
+            for k, z in enumerate(wl.z_neq):
+                Gr, sL, sR = green_dense(U, ce, co, n, z, lead_kind, wl.sr_tol, wl.sr_maxit)
+                gamL = 1j * (sL - sL.conj().T)
+                gamR = 1j * (sR - sR.conj().T)
+                GL = Gr[rows, :n]
+                GR = Gr[rows, D - n:]
+                aL = np.trace(GL @ gamL @ GL.conj().T).real
+                aR = np.trace(GR @ gamR @ GR.conj().T).real
+                out[c, k] += wgt * (fS[k] * aL + fD[k] * aR)
+    return out

@@ -25,7 +25,8 @@ STATUS_NAMES = {0: "NEGF_OK", 1: "NEGF_EINVAL", 2: "NEGF_ENOMEM", 3: "NEGF_ECUDA
 # every symbol include/negf.h declares (tests check the library exports all of them)
 EXPORTED_SYMBOLS = [
     "negf_create", "negf_destroy", "negf_set_potential", "negf_charge", "negf_transmission",
-    "negf_self_energy", "negf_current", "negf_solve_host", "negf_sync", "negf_kernel_stats", "negf_get_plan",
+    "negf_self_energy", "negf_current", "negf_set_probe", "negf_integrand_peak", "negf_solve_host", "negf_sync",
+    "negf_kernel_stats", "negf_get_plan",
     "broyden_create", "broyden_step", "broyden_reset", "broyden_destroy",
     "negf_fp64_peak", "negf_last_error", "negf_version",
 ]
@@ -89,6 +90,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
         "negf_transmission": (C.c_int, [vp, vp]),
         "negf_self_energy": (C.c_int, [vp, vp]),
         "negf_current": (C.c_int, [vp, vp, vp]),
+        "negf_set_probe": (C.c_int, [vp, i32]),
+        "negf_integrand_peak": (C.c_int, [vp, vp, vp, vp]),
         "negf_solve_host": (C.c_int, [vp, vp, vp, vp]),
         "negf_sync": (C.c_int, [vp]),
         "negf_kernel_stats": (C.c_int, [vp, C.POINTER(negf_kernel_stat), C.POINTER(i32), i32]),
@@ -218,6 +221,22 @@ class Negf:
         a = _dev_ptr(current_dev, self.C, "current_dev") if current_dev is not None else None
         b = _dev_ptr(conductance_dev, self.C, "conductance_dev") if conductance_dev is not None else None
         _check(self._lib.negf_current(self._h, a, b), "negf_current")
+
+    def negf_set_probe(self, ring: int):
+        _check(self._lib.negf_set_probe(self._h, int(ring)), "negf_set_probe")
+
+    def negf_integrand_peak(self, integrand_dev=None, k_peak_dev=None, E_peak_dev=None):
+        """integrand_dev: float64 [C][K_neq]; k_peak_dev: int32 [C]; E_peak_dev: float64 [C] (CUDA tensors or None)."""
+        import torch
+        a = _dev_ptr(integrand_dev, self.C * self.K_neq, "integrand_dev") if integrand_dev is not None else None
+        b = None
+        if k_peak_dev is not None:
+            if (not isinstance(k_peak_dev, torch.Tensor) or not k_peak_dev.is_cuda or k_peak_dev.dtype != torch.int32
+                    or not k_peak_dev.is_contiguous() or k_peak_dev.numel() < self.C):
+                raise ValueError("k_peak_dev: need a contiguous int32 CUDA tensor with >= C elements")
+            b = C.c_void_p(k_peak_dev.data_ptr())
+        c = _dev_ptr(E_peak_dev, self.C, "E_peak_dev") if E_peak_dev is not None else None
+        _check(self._lib.negf_integrand_peak(self._h, a, b, c), "negf_integrand_peak")
 
     def negf_solve_host(self, phi_host: np.ndarray, n_host: np.ndarray, T_host: Optional[np.ndarray] = None):
         """HOST buffers in, HOST buffers out (numpy arrays or pinned torch CPU tensors)."""

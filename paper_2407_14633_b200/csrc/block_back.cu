@@ -185,6 +185,8 @@ __global__ void __launch_bounds__(kBackThreads17, 2) block_back17_kernel(const S
     if (lane == 0) v += cabs2(cornv);
     v = warp_sum(v);
     if (lane == (cnt & 31)) keep = wt * v;
+    if (p.probe && (dir ? N - 1 - s : s) == p.probe_ring && lane == 0 && active)
+      p.probe[((size_t)id.c * 2 + dir) * p.K_neq + k] = wt * v;
 
     // ---- C_s becomes the B operand of the next ring
     __syncwarp();                                    // every lane has read C_{s+1}

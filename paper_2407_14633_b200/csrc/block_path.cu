@@ -272,8 +272,8 @@ negf_status block_path_self_energy(BlockPath* bp, const double* U_dev, cudaStrea
   return NEGF_OK;
 }
 
-negf_status block_path_run(BlockPath* bp, const double* U_dev, double* n_res, double* T_res,
-                           cudaStream_t s, ProfHook hook) {
+negf_status block_path_run(BlockPath* bp, const double* U_dev, double* n_res, double* T_res, int probe_ring,
+                           double* probe, cudaStream_t s, ProfHook hook) {
   blk::SweepLaunch p;
   p.C = bp->C; p.N = bp->N; p.K_eq = bp->K_eq; p.K_neq = bp->K_neq;
   p.geq = bp->geq; p.gneq = bp->gneq; p.n_eq_cta = bp->n_eq_cta;
@@ -281,6 +281,7 @@ negf_status block_path_run(BlockPath* bp, const double* U_dev, double* n_res, do
   p.table = bp->table;
   p.mu_s = bp->mu_s; p.mu_d = bp->mu_d; p.kT = bp->kT; p.deg = bp->deg; p.theta2 = bp->theta2;
   p.hist = bp->hist; p.partial = bp->partial; p.T = T_res;
+  p.probe_ring = probe_ring; p.probe = probe;
   p.csr.rowptr = bp->csr_rowptr; p.csr.col = bp->csr_col; p.csr.val = bp->csr_val;
   p.csr.nnz_cap = bp->nnz_cap;
   p.csr.diag = bp->csr_diag; p.csr.diag_mask = bp->diag_mask;

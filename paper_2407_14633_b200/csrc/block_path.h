@@ -23,8 +23,8 @@ struct ProfHook {                 // optional per-kernel timing callbacks (kinds
 negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, const double2* w_eq_dev,
                               const double2* z_neq_dev, const double* w_neq_dev, BlockPath** out);
 negf_status block_path_self_energy(BlockPath* bp, const double* U_dev, cudaStream_t s, ProfHook hook);
-negf_status block_path_run(BlockPath* bp, const double* U_dev, double* n_res, double* T_res,
-                           cudaStream_t s, ProfHook hook);
+negf_status block_path_run(BlockPath* bp, const double* U_dev, double* n_res, double* T_res, int probe_ring,
+                           double* probe, cudaStream_t s, ProfHook hook);
 negf_status block_path_check(BlockPath* bp);
 negf_status block_path_copy_sigma(BlockPath* bp, double2* sigma_dev, cudaStream_t s);
 void block_path_plan(BlockPath* bp, negf_plan_info* out);
@@ -81,6 +81,8 @@ struct SweepLaunch {
   double2* hist;              // [slots][N][2 row slots][nb][THREADS]
   double* partial;            // [C][geq + 2 gneq][N]
   double* T;                  // [C][K_neq]
+  int probe_ring;             // >= 0: ring whose per-energy charge contributions are recorded
+  double* probe;              // [C][2 directions][K_neq], or nullptr
   CsrSet csr;
 };
 cudaError_t launch_block_sweep(int nb, const SweepLaunch& p, cudaStream_t s);

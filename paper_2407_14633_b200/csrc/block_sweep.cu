@@ -359,6 +359,15 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
 #pragma unroll
     for (int b = 0; b < NB; ++b) v += cabs2(cc[0][b]) + cabs2(cc[1][b]);
     v = live ? wt * v : 0.0;
+    if (p.probe && i == p.probe_ring) {                            // per-task value (CTA-uniform branch)
+      if (live) sm.mag[t * NB + a] = v;
+      __syncthreads();
+      if (a == 0 && active) {
+        double tot = 0.0;
+        for (int r = 0; r < TPT; ++r) tot += sm.mag[t * NB + r];
+        p.probe[((size_t)id.c * 2 + dir) * p.K_neq + k] = tot;
+      }
+    }
     v = warp_sum(v);
     if (lane == 0) sm.red[(s & 1) * G::NWARPS + warp] = v;
     __syncthreads();

@@ -69,6 +69,9 @@ struct negf_handle {
   double *n_res, *T_res;
   // host staging for negf_solve_host
   double* phi_stage;        // device [C][N]
+  // probe ring of the semi-adaptive real-axis path
+  int probe_ring;           // -1: off
+  double* probe;            // [C][2][n_modes][K_neq]
   // block path
   BlockPath* block;
   // profiling
@@ -213,6 +216,7 @@ negf_status run_sweeps(negf_handle* h) {
     p.hist_c = reinterpret_cast<double2*>(h->hist);
     p.partial = h->partial; p.T_part = h->T_part;
     p.side = h->side; p.ev_fork = h->ev_fork; p.ev_join = h->ev_join;
+    p.probe_ring = h->probe_ring; p.probe = h->probe_ring >= 0 ? h->probe : nullptr;
     for (const Batch& b : h->batches) {
       p.warp_begin = b.warp_begin;
       p.warp_end = b.warp_end;
@@ -227,7 +231,8 @@ negf_status run_sweeps(negf_handle* h) {
       NEGF_CUDA_TRY(launch_reduce_modes(h->T_part, h->T_res, h->C, h->n_modes, h->K_neq, h->stream));
     }
   } else {
-    negf_status st = block_path_run(h->block, h->U, h->n_res, h->T_res, h->stream, prof_hook(h));
+    negf_status st = block_path_run(h->block, h->U, h->n_res, h->T_res, h->probe_ring,
+                                    h->probe_ring >= 0 ? h->probe : nullptr, h->stream, prof_hook(h));
     if (st != NEGF_OK) return st;
   }
   h->results_valid = true;
@@ -247,7 +252,7 @@ extern "C" negf_status negf_destroy(negf_handle* h) {
   cudaFree(h->z_eq); cudaFree(h->w_eq); cudaFree(h->z_neq); cudaFree(h->w_neq);
   cudaFree(h->bsq_even); cudaFree(h->bsq_odd); cudaFree(h->mode_w); cudaFree(h->mode_w_T);
   cudaFree(h->U); cudaFree(h->hist); cudaFree(h->partial); cudaFree(h->scratch);
-  cudaFree(h->T_part); cudaFree(h->n_res); cudaFree(h->T_res); cudaFree(h->phi_stage);
+  cudaFree(h->T_part); cudaFree(h->n_res); cudaFree(h->T_res); cudaFree(h->phi_stage); cudaFree(h->probe);
   if (h->block) block_path_destroy(h->block);
   if (h->side) cudaStreamDestroy(h->side);
   if (h->ev_fork) cudaEventDestroy(h->ev_fork);
@@ -302,6 +307,7 @@ extern "C" negf_status negf_create(const negf_config* cfg, void* cuda_stream, ne
   h->K_eq = cfg->n_eq; h->K_neq = cfg->n_neq;
   h->scalar = scalar;
   h->profile = cfg->profile != 0;
+  h->probe_ring = -1;
 
   auto fail = [&](negf_status st) { negf_destroy(h); return st; };
   cudaError_t e = cudaSuccess;
@@ -397,6 +403,32 @@ extern "C" negf_status negf_current(negf_handle* h, double* current_dev, double*
   ProfScope ps(h, K_MISC);
   NEGF_CUDA_TRY(launch_landauer(h->T_res, h->z_neq, h->w_neq, h->C, h->K_neq, h->cfg.mu_s, h->cfg.mu_d,
                                 h->cfg.kT, current_dev, conductance_dev, h->stream));
+  return NEGF_OK;
+}
+
+extern "C" negf_status negf_set_probe(negf_handle* h, int32_t ring) {
+  if (!h) { set_error("negf_set_probe: null handle"); return NEGF_EINVAL; }
+  if (ring >= h->N) { set_error("negf_set_probe: ring %d outside [0, %d)", ring, h->N); return NEGF_EINVAL; }
+  if (ring >= 0 && h->K_neq < 1) { set_error("negf_set_probe: the handle has no real-axis points"); return NEGF_EINVAL; }
+  if (ring >= 0 && !h->probe) {
+    const size_t cnt = (size_t)h->C * 2 * h->n_modes * h->K_neq;
+    NEGF_CUDA_TRY(cudaMalloc((void**)&h->probe, sizeof(double) * cnt));
+    NEGF_CUDA_TRY(cudaMemsetAsync(h->probe, 0, sizeof(double) * cnt, h->stream));
+  }
+  h->probe_ring = ring < 0 ? -1 : ring;
+  h->results_valid = false;
+  return NEGF_OK;
+}
+
+extern "C" negf_status negf_integrand_peak(negf_handle* h, double* integrand_dev, int32_t* k_peak_dev,
+                                           double* E_peak_dev) {
+  if (!h) { set_error("negf_integrand_peak: null handle"); return NEGF_EINVAL; }
+  if (h->probe_ring < 0) { set_error("negf_integrand_peak: no probe ring set (negf_set_probe)"); return NEGF_ESTATE; }
+  negf_status st = run_sweeps(h);
+  if (st != NEGF_OK) return st;
+  ProfScope ps(h, K_MISC);
+  NEGF_CUDA_TRY(launch_integrand_peak(h->probe, h->C, h->n_modes, h->K_neq, h->z_neq, h->w_neq, h->cfg.deg,
+                                      integrand_dev, k_peak_dev, E_peak_dev, h->stream));
   return NEGF_OK;
 }
 

@@ -42,6 +42,8 @@ struct ScalarLaunch {
   double2* hist_c;          // contour history:   [warp][N][32] double2
   double* partial;          // [total warps][N] per-warp partial charge
   double* T_part;           // [C][n_modes][K_neq]
+  int probe_ring;           // >= 0: ring whose per-energy charge contributions are recorded
+  double* probe;            // [C][2 directions][n_modes][K_neq], or nullptr
   int warp_begin, warp_end; // global warp range of this launch
   cudaStream_t side;        // host only: stream of the contour kernel (forked from / joined to s)
   cudaEvent_t ev_fork, ev_join;
@@ -57,6 +59,11 @@ cudaError_t launch_reduce_modes(const double* T_part, double* T, int C, int n_mo
                                 cudaStream_t s);
 cudaError_t launch_negate(const double* in, double* out, int64_t n, cudaStream_t s);
 // current / conductance reductions of T(E)  (eq.(5)-(6))
+// Integrand of the real-axis part of eq.(4) at the probe ring and its peak:
+// integrand[c][k] = 2 pi / (deg w_k) * sum_{dir, mode} probe[c][dir][mode][k]; k_peak[c] = first arg-max over k.
+cudaError_t launch_integrand_peak(const double* probe, int C, int n_modes, int K, const double2* z_neq,
+                                  const double* w_neq, double deg, double* integrand, int* k_peak,
+                                  double* E_peak, cudaStream_t s);
 cudaError_t launch_landauer(const double* T, const double2* z_neq, const double* w_neq, int C, int K,
                             double mu_s, double mu_d, double kT, double* current,
                             double* conductance, cudaStream_t s);

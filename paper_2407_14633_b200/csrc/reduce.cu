@@ -92,7 +92,54 @@ __global__ void landauer_kernel(const double* __restrict__ T, const double2* __r
   }
 }
 
+// the integrand A_1 F_1 + A_2 F_2 of eq.(4) at the probe ring as a function of
+// energy, and the position of its peak.  One block per channel; the arg-max is the FIRST maximum (fixed-order
+// tree with index tie-break), so the result is deterministic.
+__global__ void integrand_peak_kernel(const double* __restrict__ probe, int n_modes, int K,
+                                      const double2* __restrict__ z, const double* __restrict__ w, double deg,
+                                      double* __restrict__ integrand, int* __restrict__ k_peak,
+                                      double* __restrict__ E_peak) {
+  __shared__ double sv[256];
+  __shared__ int si[256];
+  const int c = blockIdx.x;
+  const double* pc = probe + (size_t)c * 2 * n_modes * K;
+  double best = -1.0;
+  int bi = 0x7fffffff;
+  for (int k = threadIdx.x; k < K; k += 256) {
+    double acc = 0.0;
+    for (int dm = 0; dm < 2 * n_modes; ++dm) acc += pc[(size_t)dm * K + k];
+    const double val = acc * (2.0 * 3.14159265358979323846) / (deg * w[k]);
+    if (integrand) integrand[(size_t)c * K + k] = val;
+    if (val > best) { best = val; bi = k; }                 // k increases: keeps the first maximum of this thread
+  }
+  sv[threadIdx.x] = best;
+  si[threadIdx.x] = bi;
+  __syncthreads();
+  for (int h = 128; h > 0; h >>= 1) {
+    if (threadIdx.x < h) {
+      const double ov = sv[threadIdx.x + h];
+      const int oi = si[threadIdx.x + h];
+      if (ov > sv[threadIdx.x] || (ov == sv[threadIdx.x] && oi < si[threadIdx.x])) {
+        sv[threadIdx.x] = ov;
+        si[threadIdx.x] = oi;
+      }
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    if (k_peak) k_peak[c] = si[0];
+    if (E_peak) E_peak[c] = z[si[0]].x;
+  }
+}
+
 }  // namespace
+
+cudaError_t launch_integrand_peak(const double* probe, int C, int n_modes, int K, const double2* z_neq,
+                                  const double* w_neq, double deg, double* integrand, int* k_peak,
+                                  double* E_peak, cudaStream_t s) {
+  integrand_peak_kernel<<<C, 256, 0, s>>>(probe, n_modes, K, z_neq, w_neq, deg, integrand, k_peak, E_peak);
+  return cudaGetLastError();
+}
 
 cudaError_t launch_reduce_rows(const double* in, double* out, int n_out, int rows_per_out, int cols,
                                double scale, double* scratch, cudaStream_t s) {

@@ -239,6 +239,10 @@ scalar_real_kernel(const ScalarLaunch p, const int n_warps) {
     const double* __restrict__ hrd = hist + (size_t)(N - 1) * 32;   // walks down the history
     double g2 = 0.0;
     int q0 = 0;
+    // probe: way-back position of the ring whose per-energy contributions are recorded
+    const int probe_pos = (p.probe_ring >= 0 && p.probe) ? sign * (p.probe_ring - ring0) : -1;
+    double* __restrict__ probe_out =
+        p.probe ? p.probe + (((size_t)c * 2 + dir) * p.n_modes + mode) * p.K_neq + k : nullptr;
     for (; q0 + kTile <= N; q0 += kTile, hrd -= (size_t)kTile * 32) {   // full tiles: no tail tests
       double h[kTile];
 #pragma unroll
@@ -250,6 +254,7 @@ scalar_real_kernel(const ScalarLaunch p, const int n_warps) {
         if (__double2hiint(h[t]) < 0) c2 = cross_marker(c2, h[t]);   // rare: a rescaled step
         c2 *= (t & 1) ? b2_t_odd : b2_t_even;
       }
+      if ((unsigned)(probe_pos - q0) < (unsigned)kTile && active) *probe_out = tile[probe_pos - q0][lane];
       flush_tile(tile, lane, kTile, prow, ring0 + sign * q0, sign);
     }
     if (q0 < N) {                                          // ragged last tile
@@ -266,6 +271,7 @@ scalar_real_kernel(const ScalarLaunch p, const int n_warps) {
         }
         tile[t][lane] = v;
       }
+      if ((unsigned)(probe_pos - q0) < (unsigned)cnt && active) *probe_out = tile[probe_pos - q0][lane];
       flush_tile(tile, lane, cnt, prow, ring0 + sign * q0, sign);
     }
     // the last value is |G_(first,last)|^2: transmission through the chain (eq.(5)), a4

@@ -258,3 +258,39 @@ def test_table2_long_channel_workload():
     n_sub = gpu_charge(sub)
     n_ref, _ = omp.charge_and_transmission(sub)
     assert_parity(n_sub, n_ref, "table2 full-length charge of sampled chains, every ring")
+
+
+@pytest.mark.parametrize("cfg,kw,ring", [(2, dict(N=37, K_neq=45, K_eq=4), 18), (2, dict(N=37, K_neq=45, K_eq=4), 0),
+                                         (1, dict(N=30, K_neq=33), 29), (3, dict(N=9, K_neq=10, K_eq=2), 4),
+                                         (4, dict(C=2, N=8, K_neq=9, K_eq=2), 7)])
+def test_integrand_probe_and_peak_vs_definition(cfg, kw, ring):
+    """SURVEY 8(f)-2, device side: the integrand A_1 F_1 + A_2 F_2 at a probe ring as a function
+    of energy and the position of its peak, against the dense definition; the charge must not depend on
+    the probe; the host-side refresh then puts the dense segment around the peak."""
+    import torch
+    from paper_2407_14633_b200 import Negf
+    wl = wlmod.make_config(cfg, **kw)
+    I_ref = od.integrand_dense(wl, ring)
+    h = Negf.from_workload(wl)
+    phi = torch.tensor(wl.phi, dtype=torch.float64, device="cuda")
+    n0 = torch.empty((wl.C, wl.N), dtype=torch.float64, device="cuda")
+    n1 = torch.empty_like(n0)
+    h.negf_set_potential(phi)
+    h.negf_charge(n0)
+    h.negf_set_probe(ring)
+    h.negf_charge(n1)
+    I = torch.empty((wl.C, wl.K_neq), dtype=torch.float64, device="cuda")
+    kp = torch.empty(wl.C, dtype=torch.int32, device="cuda")
+    Ep = torch.empty(wl.C, dtype=torch.float64, device="cuda")
+    h.negf_integrand_peak(I, kp, Ep)
+    h.negf_sync()
+    assert torch.equal(n0, n1)                                        # the probe does not touch the charge
+    assert_parity(I.cpu().numpy(), I_ref, f"config{cfg} integrand at ring {ring}")
+    assert np.array_equal(kp.cpu().numpy(), np.argmax(I_ref, axis=1))
+    assert np.array_equal(Ep.cpu().numpy(), wl.z_neq.real[np.argmax(I_ref, axis=1)])
+    e_s, l1, l2 = wlmod.refine_segment_limits(wl.z_neq.real, I.cpu().numpy()[0], wl.kT)
+    assert e_s == Ep.cpu().numpy()[0] and l1 < e_s < l2
+    h.negf_set_probe(-1)
+    with pytest.raises(Exception):
+        h.negf_integrand_peak(I, kp, Ep)
+    h.negf_destroy()

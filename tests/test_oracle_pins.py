@@ -474,6 +474,23 @@ def test_f2_refine_segment_limits_brackets_the_peak():
     assert abs(e_s + 0.2713) < 1e-3 and l1 == e_s - 3 * 0.0259 and l2 == e_s + 0.0259
 
 
+def test_f2_integrand_sums_to_the_real_axis_charge():
+    """integrand_dense is the energy-resolved second term of eq.(4): deg/(2 pi) sum_k w_k I(E_k) must give the
+    real-axis charge of that ring; for the ideal tube deep in a band it equals 2 pi x the local density
+    of states summed over the open modes times the occupation (A_S + A_D = 2 pi LDOS, P5)."""
+    w = wlmod.make_config(2, N=11, K_neq=14, K_eq=0)
+    I = od.integrand_dense(w, 5)
+    n, _ = od.charge_and_transmission(w)
+    assert abs(w.deg / (2 * np.pi) * np.sum(w.w_neq * I[0]) - n[0, 5]) < 1e-13 * n[0, 5]
+    # ideal uniform chain, E inside the band, both leads fully occupied: A_S + A_D = 2 pi LDOS = 2 / sqrt(4t^2 - E^2)
+    c = wlmod.make_config(1, N=9, K_neq=5)
+    c.phi[:] = 0.0
+    c.mu_s = c.mu_d = 50.0
+    c.z_neq = (np.array([-1.0, -0.3, 0.0, 0.4, 2.0]) + 1e-9j).astype(np.complex128)
+    I = od.integrand_dense(c, 4)
+    assert np.max(np.abs(I[0] - 2.0 / np.sqrt(4 * 2.5 ** 2 - c.z_neq.real ** 2))) < 1e-7
+
+
 # ------------------------------------------------------------------ P10: brute force, O1 vs O3
 
 def _random_hermitian_device(rng, N, n):
