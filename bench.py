@@ -439,9 +439,12 @@ def run_ours(args):
             if c == 1:
                 entry["note"] = "1000 sweeps of 100 sites: launch-latency-bound (SURVEY 8(d)); parity / smoke config"
             if c == 6:
-                entry["note"] = ("N = 524 288 rings, 90 contour points, 8 modes: 1440 half-sweep chains, each a serial "
-                                 "pass over all rings -- latency-bound (45 warps on 148 SMs); the paper's own time for this "
-                                 "shape is 5.63 s (Table 2, PAPER.md:333; GPU count not stated)")
+                entry["note"] = ("N = 524 288 rings, 90 contour points, 8 modes: 1440 half-sweep chains run PARALLEL IN N "
+                                 "(1024 segments of 512 rings: segment transfer products, serial pass over the segment "
+                                 "starts, parallel re-run; scalar_sweep.cu); the serial pass of the same kernels takes 84 ms; "
+                                 "the paper's own time for this shape is 5.63 s (Table 2, PAPER.md:333; GPU count not stated). "
+                                 "The history actually written and re-read is 64 B per ring and chain pair (two 16-byte "
+                                 "directions), twice the 32 B SURVEY 8(d) counts")
             if c == 5:
                 entry["note"] = ("one step = one Broyden iteration of the 20-iteration loop (history 8, mixing 0.1); "
                                  "the full loop is 20 x ms_per_step")

@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -43,6 +44,14 @@ struct Batch {
   int warp_begin, warp_end;
 };
 
+// scalar handles with at least this many rings run their contour half-sweeps parallel in N (the
+// environment variables NEGF_SEG_MIN_RINGS / NEGF_SEG_LEN override the threshold / the segment length, read at
+// negf_create; the tests use them to exercise the path on short devices and to compare with the serial pass)
+int seg_min_rings() {
+  const char* e = getenv("NEGF_SEG_MIN_RINGS");
+  return e ? atoi(e) : 8192;
+}
+
 }  // namespace
 
 struct negf_handle {
@@ -63,6 +72,8 @@ struct negf_handle {
   char* hist;
   int64_t hist_bytes, partial_bytes;
   double *partial, *scratch, *T_part;
+  double2 *seg_M, *seg_v;   // parallel-in-N contour path (long channels), else nullptr
+  int seg_S, seg_L;
   cudaStream_t side;        // contour tasks run beside the real-axis tasks (fork / join by events)
   cudaEvent_t ev_fork, ev_join;
   // results
@@ -190,6 +201,24 @@ negf_status plan_scalar(negf_handle* h) {
   NEGF_CUDA_TRY(cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking));
   NEGF_CUDA_TRY(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
   NEGF_CUDA_TRY(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
+  // Long channels: the contour half-sweeps are cut into segments of >= 256 steps and run parallel in N
+  // (scalar_sweep.cu).  Workspace: 6 complex per (task, segment).
+  h->seg_M = h->seg_v = nullptr;
+  h->seg_S = h->seg_L = 0;
+  if (N >= seg_min_rings() && N >= 3 && h->cwarps_per_channel > 0) {
+    const char* le = getenv("NEGF_SEG_LEN");             // test hook: segment length
+    h->seg_L = le ? std::max(1, atoi(le)) : (int)std::max<int64_t>(256, (N - 1 + 1023) / 1024);
+    h->seg_S = (int)((N - 1 + h->seg_L - 1) / h->seg_L);
+    int max_cw = 0;                                       // most contour warps in one batch
+    for (const Batch& b : h->batches) {
+      int cw = 0;
+      for (int w = b.warp_begin; w < b.warp_end; ++w) cw += (w % wpc) < h->cwarps_per_channel;
+      max_cw = std::max(max_cw, cw);
+    }
+    const size_t per = (size_t)max_cw * h->seg_S * 32;
+    NEGF_CUDA_TRY(cudaMalloc((void**)&h->seg_M, sizeof(double2) * 4 * per));
+    NEGF_CUDA_TRY(cudaMalloc((void**)&h->seg_v, sizeof(double2) * 2 * per));
+  }
   const int nslice = (wpc + 63) / 64;
   NEGF_CUDA_TRY(cudaMalloc((void**)&h->scratch, sizeof(double) * (size_t)h->C * nslice * N));
   NEGF_CUDA_TRY(cudaMalloc((void**)&h->T_part,
@@ -217,6 +246,7 @@ negf_status run_sweeps(negf_handle* h) {
     p.partial = h->partial; p.T_part = h->T_part;
     p.side = h->side; p.ev_fork = h->ev_fork; p.ev_join = h->ev_join;
     p.probe_ring = h->probe_ring; p.probe = h->probe_ring >= 0 ? h->probe : nullptr;
+    p.seg_M = h->seg_M; p.seg_v = h->seg_v; p.seg_S = h->seg_S; p.seg_L = h->seg_L;
     for (const Batch& b : h->batches) {
       p.warp_begin = b.warp_begin;
       p.warp_end = b.warp_end;
@@ -252,6 +282,7 @@ extern "C" negf_status negf_destroy(negf_handle* h) {
   cudaFree(h->z_eq); cudaFree(h->w_eq); cudaFree(h->z_neq); cudaFree(h->w_neq);
   cudaFree(h->bsq_even); cudaFree(h->bsq_odd); cudaFree(h->mode_w); cudaFree(h->mode_w_T);
   cudaFree(h->U); cudaFree(h->hist); cudaFree(h->partial); cudaFree(h->scratch);
+  cudaFree(h->seg_M); cudaFree(h->seg_v);
   cudaFree(h->T_part); cudaFree(h->n_res); cudaFree(h->T_res); cudaFree(h->phi_stage); cudaFree(h->probe);
   if (h->block) block_path_destroy(h->block);
   if (h->side) cudaStreamDestroy(h->side);
@@ -491,7 +522,7 @@ extern "C" negf_status negf_get_plan(negf_handle* h, negf_plan_info* out) {
       bool has_c = false, has_r = false;
       for (int w = b.warp_begin; w < b.warp_end && !(has_c && has_r); ++w)
         ((w % wpc) < h->cwarps_per_channel ? has_c : has_r) = true;
-      launches += (has_r ? 1 : 0) + (has_c ? 2 : 0);
+      launches += (has_r ? 1 : 0) + (has_c ? (h->seg_M ? 4 : 2) : 0);
     }
     out->kernel_launches = launches;
   } else {

@@ -44,6 +44,10 @@ struct ScalarLaunch {
   double* T_part;           // [C][n_modes][K_neq]
   int probe_ring;           // >= 0: ring whose per-energy charge contributions are recorded
   double* probe;            // [C][2 directions][n_modes][K_neq], or nullptr
+  // parallel-in-N contour path (scalar_sweep.cu): steps 1 .. N-1 in seg_S segments of seg_L steps; nullptr = serial
+  double2* seg_M;           // [contour warp of the launch][segment][4 components][32 lanes]
+  double2* seg_v;           // [contour warp of the launch][segment][2 components][32 lanes]
+  int seg_S, seg_L;
   int warp_begin, warp_end; // global warp range of this launch
   cudaStream_t side;        // host only: stream of the contour kernel (forked from / joined to s)
   cudaEvent_t ev_fork, ev_join;

@@ -280,86 +280,194 @@ scalar_real_kernel(const ScalarLaunch p, const int n_warps) {
   }
 }
 
-__global__ void __launch_bounds__(kWarpsPerBlock * 32, 8)
-scalar_contour_kernel(const ScalarLaunch p, const int n_warps) {
-  __shared__ double tiles[kWarpsPerBlock][kTile][33];
-  const int lane = threadIdx.x & 31;
-  const int wib = threadIdx.x >> 5;
-  const int ord = blockIdx.x * kWarpsPerBlock + wib;      // ordinal among this launch's contour warps
-  if (ord >= n_warps) return;
-  double(*tile)[33] = tiles[wib];
+// ---------------------------------------------------------------------------------- contour tasks
+// One contour half-sweep task = (channel, mode, contour point, direction); a warp holds 32 of them.
+// Direction 0 stores y_i (left-connected), direction 1 stores x_i (right-connected), both indexed by
+// ring; scalar_combine_kernel then forms G_(i,i) (Alg.1 step 1).
+struct ContourTask {
+  int N, dir, istep, i0;
+  cplx z, sig_first;
+  double b2_odd_s, b2_even_s;       // |bond|^2 entering odd / even steps s
+  const double* U;                  // on-site energies of the task's channel
+  double2* hist;                    // [ring][32 lanes], already offset by the lane
+};
 
+__device__ __forceinline__ ContourTask contour_task(const ScalarLaunch& p, int ord, int lane) {
+  ContourTask t;
   const int N = p.N;
   const int wpc = p.cwarps_per_channel + 2 * p.rwarps_per_channel;
   auto cw_before = [&](int ww) { return (ww / wpc) * p.cwarps_per_channel + min(ww % wpc, p.cwarps_per_channel); };
   const int cw0 = cw_before(p.warp_begin);
   const int g = cw0 + ord;                                // global contour warp ordinal
   const int c = g / p.cwarps_per_channel;
-  const int local = g - c * p.cwarps_per_channel;
+  const int local = g - c * p.cwarps_per_channel;         // = 2 * group + direction
   const int w = c * wpc + local;                          // global warp index
-  const double* __restrict__ U = p.U + (size_t)c * N;
-  double* __restrict__ prow = p.partial + (size_t)w * N;
+  t.N = N;
+  t.U = p.U + (size_t)c * N;
   // history offset of this warp inside the launch's workspace
   const long long cwb = cw_before(w) - cw0;
   const long long rwb = (long long)(w - p.warp_begin) - cwb;
   char* hbase = reinterpret_cast<char*>(p.hist_r) + (cwb * 16 + rwb * 8) * (long long)N * 32;
-  const double U0 = __ldg(U), UN = __ldg(U + N - 1);
-  {
-    // ------------------------------------------------------------------ contour half-sweep task
-    // local = 2 * group + direction.  Direction 0 stores y_i (left-connected), direction 1 stores x_i
-    // (right-connected), both indexed by ring; scalar_combine_kernel then forms G_(i,i) (Alg.1 step 1).
-    (void)tile; (void)prow;
-    const int dir = local & 1;
-    const int grp = local >> 1;
-    const int ntask = p.n_modes * p.K_eq;
-    int e = grp * 32 + lane;
-    if (e >= ntask) e = ntask - 1;
-    const int mode = e / p.K_eq;
-    const int k = e - mode * p.K_eq;
-    const cplx z = {p.z_eq[k].x, p.z_eq[k].y};
-    const double be = __ldg(p.bsq_even + mode), bo = __ldg(p.bsq_odd + mode);
-    cplx sig_first;
-    if (dir == 0) {
-      const cplx gl = surface_gf_alternating({z.re - U0, z.im}, sqrt(be), sqrt(bo));
-      sig_first = {bo * gl.re, bo * gl.im};
-    } else {
-      const double tauR2 = ((N - 1) & 1) ? bo : be, t1R2 = ((N - 1) & 1) ? be : bo;
-      const cplx gr = surface_gf_alternating({z.re - UN, z.im}, sqrt(t1R2), sqrt(tauR2));
-      sig_first = {tauR2 * gr.re, tauR2 * gr.im};
-    }
-    double2* __restrict__ hist = reinterpret_cast<double2*>(hbase) + lane;
-    const int par0 = dir ? ((N - 1) & 1) : 1;       // bond type entering step s is par0 ^ (s & 1)
-    const double b2_odd_s = par0 ? be : bo;
-    const double b2_even_s = par0 ? bo : be;
-    const int istep = dir ? -1 : 1;
-    int i = dir ? N - 1 : 0;
-    // Homogeneous form of Alg.2 (see scalar_real_kernel): P_{s+1} = alpha_s P_s - b2_s P_{s-1} keeps the
-    // dependent chain free of divisions; the stored quantity y_s = b2_s g_{s-1} = b2_s P_{s-1} / P_s
-    // (x_i for direction 1) is formed off the chain and is invariant under the power-of-two rescaling.
-    hist[(size_t)i * 32] = make_double2(sig_first.re, sig_first.im);   // the lead plays ring "-1"
-    double qr = 1.0, qi = 0.0;                                          // P_0
-    double pr = z.re - __ldg(U + i) - sig_first.re, pi_ = z.im - sig_first.im;   // P_1
-    i += istep;
-    for (int s = 1; s < N; ++s, i += istep) {
-      const double b2 = (s & 1) ? b2_odd_s : b2_even_s;
-      // y_s = b2 P_{s-1} conj(P_s) / |P_s|^2
-      const double m = fma(pr, pr, pi_ * pi_);
-      const double r = b2 / m;
-      const double tr = fma(qr, pr, qi * pi_), ti = fma(qi, pr, -qr * pi_);
-      hist[(size_t)i * 32] = make_double2(tr * r, ti * r);
-      const double ar = z.re - __ldg(U + i);
-      double nr = fma(ar, pr, fma(-z.im, pi_, -b2 * qr));
-      double ni = fma(ar, pi_, fma(z.im, pr, -b2 * qi));
-      qr = pr; qi = pi_; pr = nr; pi_ = ni;
-      if ((s & 3) == 0) {
-        const unsigned ex = (unsigned)(__double2hiint(m) >> 20) - 623u;
-        if (ex > 800u && m > 0.0) {
-          const double sc = (ex < 0x80000000u) ? 0x1p-200 : 0x1p200;
-          pr *= sc; pi_ *= sc; qr *= sc; qi *= sc;
-        }
+  t.hist = reinterpret_cast<double2*>(hbase) + lane;
+  t.dir = local & 1;
+  const int grp = local >> 1;
+  const int ntask = p.n_modes * p.K_eq;
+  int e = grp * 32 + lane;
+  if (e >= ntask) e = ntask - 1;
+  const int mode = e / p.K_eq;
+  const int k = e - mode * p.K_eq;
+  t.z = {p.z_eq[k].x, p.z_eq[k].y};
+  const double be = __ldg(p.bsq_even + mode), bo = __ldg(p.bsq_odd + mode);
+  if (t.dir == 0) {
+    const cplx gl = surface_gf_alternating({t.z.re - __ldg(t.U), t.z.im}, sqrt(be), sqrt(bo));
+    t.sig_first = {bo * gl.re, bo * gl.im};
+  } else {
+    const double tauR2 = ((N - 1) & 1) ? bo : be, t1R2 = ((N - 1) & 1) ? be : bo;
+    const cplx gr = surface_gf_alternating({t.z.re - __ldg(t.U + N - 1), t.z.im}, sqrt(t1R2), sqrt(tauR2));
+    t.sig_first = {tauR2 * gr.re, tauR2 * gr.im};
+  }
+  const int par0 = t.dir ? ((N - 1) & 1) : 1;       // bond type entering step s is par0 ^ (s & 1)
+  t.b2_odd_s = par0 ? be : bo;
+  t.b2_even_s = par0 ? bo : be;
+  t.istep = t.dir ? -1 : 1;
+  t.i0 = t.dir ? N - 1 : 0;
+  return t;
+}
+
+// Steps s = s0 .. s1-1 of the homogeneous form of Alg.2 (see scalar_real_kernel): on entry (pr, pi_) = P_s0,
+// (qr, qi) = P_{s0-1}; every step stores y_s = b2_s g_{s-1} = b2_s P_{s-1} / P_s (x_i for direction 1) at its
+// ring -- formed off the dependent chain and invariant under the power-of-two rescaling -- and advances
+// P_{s+1} = alpha_s P_s - b2_s P_{s-1}.
+__device__ __forceinline__ void contour_steps(const ContourTask& t, int s0, int s1, double& pr, double& pi_,
+                                              double& qr, double& qi) {
+  int i = t.i0 + t.istep * s0;
+  for (int s = s0; s < s1; ++s, i += t.istep) {
+    const double b2 = (s & 1) ? t.b2_odd_s : t.b2_even_s;
+    // y_s = b2 P_{s-1} conj(P_s) / |P_s|^2
+    const double m = fma(pr, pr, pi_ * pi_);
+    const double r = b2 / m;
+    const double tr = fma(qr, pr, qi * pi_), ti = fma(qi, pr, -qr * pi_);
+    t.hist[(size_t)i * 32] = make_double2(tr * r, ti * r);
+    const double ar = t.z.re - __ldg(t.U + i);
+    double nr = fma(ar, pr, fma(-t.z.im, pi_, -b2 * qr));
+    double ni = fma(ar, pi_, fma(t.z.im, pr, -b2 * qi));
+    qr = pr; qi = pi_; pr = nr; pi_ = ni;
+    if ((s & 3) == 0) {
+      const unsigned ex = (unsigned)(__double2hiint(m) >> 20) - 623u;
+      if (ex > 800u && m > 0.0) {
+        const double sc = (ex < 0x80000000u) ? 0x1p-200 : 0x1p200;
+        pr *= sc; pi_ *= sc; qr *= sc; qi *= sc;
       }
     }
   }
+}
+
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 8)
+scalar_contour_kernel(const ScalarLaunch p, const int n_warps) {
+  const int lane = threadIdx.x & 31;
+  const int ord = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);   // ordinal among this launch's contour warps
+  if (ord >= n_warps) return;
+  const ContourTask t = contour_task(p, ord, lane);
+  t.hist[(size_t)t.i0 * 32] = make_double2(t.sig_first.re, t.sig_first.im);   // the lead plays ring "-1"
+  double qr = 1.0, qi = 0.0;                                                   // P_0
+  double pr = t.z.re - __ldg(t.U + t.i0) - t.sig_first.re, pi_ = t.z.im - t.sig_first.im;   // P_1
+  contour_steps(t, 1, t.N, pr, pi_, qr, qi);
+}
+
+// ---------------------------------------------------------------------------------- parallel in N
+// Long channels with few contour points (the shape of the paper's Table 2: N = 524 288 rings, 90 points,
+// PAPER.md:325-335) leave the serial pass above with a few dozen warps.  The recursion is
+// linear in (P_s, P_{s-1}),  [P_{s+1}; P_s] = T_s [P_s; P_{s-1}],  T_s = [[alpha_s, -b2_s], [1, 0]],  so the
+// steps 1 .. N-1 are cut into S segments of L steps and done in three passes:
+//   A  (parallel over tasks x segments)  M_m = product of the segment's T_s, as the images of the two unit
+//      vectors, with one common power-of-two rescaling (only ratios of P are ever used);
+//   B  (parallel over tasks, serial over the S segments)  the state at every segment start, v_{m+1} = M_m v_m;
+//   C  (parallel over tasks x segments)  the very steps of the serial kernel from the segment's start state.
+// Pass C computes every stored y_s by the same recurrence as the serial kernel; the segment start states
+// differ from the serial ones only by the rounding of the 2 x 2 products.  For Im z > 0 the forward recursion
+// is dominated by its growing solution, so M_m v_m has no cancellation.  (This is NOT the transfer-matrix
+// scan of |G| on the real axis that SURVEY 7 warns about: only the contour tasks use it.)
+__device__ __forceinline__ void seg_range(const ScalarLaunch& p, int m, int& s0, int& s1) {
+  s0 = 1 + m * p.seg_L;
+  s1 = min(s0 + p.seg_L, p.N);
+}
+
+__global__ void __launch_bounds__(128, 8) scalar_contour_segA_kernel(const ScalarLaunch p, const int n_warps) {
+  const int lane = threadIdx.x & 31;
+  const long long job = (long long)blockIdx.x * 4 + (threadIdx.x >> 5);
+  const int ord = (int)(job / p.seg_S), m = (int)(job - (long long)ord * p.seg_S);
+  if (ord >= n_warps) return;
+  const ContourTask t = contour_task(p, ord, lane);
+  int s0, s1;
+  seg_range(p, m, s0, s1);
+  // columns of M_m: start states (P_s0, P_{s0-1}) = (1, 0) and (0, 1)
+  double ar_ = 1.0, ai_ = 0.0, br_ = 0.0, bi_ = 0.0;      // first column: P_s, P_{s-1}
+  double cr_ = 0.0, ci_ = 0.0, dr_ = 1.0, di_ = 0.0;      // second column
+  int i = t.i0 + t.istep * s0;
+  for (int s = s0; s < s1; ++s, i += t.istep) {
+    const double b2 = (s & 1) ? t.b2_odd_s : t.b2_even_s;
+    const double al = t.z.re - __ldg(t.U + i);
+    const double n1r = fma(al, ar_, fma(-t.z.im, ai_, -b2 * br_)), n1i = fma(al, ai_, fma(t.z.im, ar_, -b2 * bi_));
+    const double n2r = fma(al, cr_, fma(-t.z.im, ci_, -b2 * dr_)), n2i = fma(al, ci_, fma(t.z.im, cr_, -b2 * di_));
+    br_ = ar_; bi_ = ai_; ar_ = n1r; ai_ = n1i;
+    dr_ = cr_; di_ = ci_; cr_ = n2r; ci_ = n2i;
+    if ((s & 3) == 0) {
+      const double mm = fmax(fma(ar_, ar_, ai_ * ai_), fma(cr_, cr_, ci_ * ci_));
+      const unsigned ex = (unsigned)(__double2hiint(mm) >> 20) - 623u;
+      if (ex > 800u && mm > 0.0) {
+        const double sc = (ex < 0x80000000u) ? 0x1p-200 : 0x1p200;
+        ar_ *= sc; ai_ *= sc; br_ *= sc; bi_ *= sc; cr_ *= sc; ci_ *= sc; dr_ *= sc; di_ *= sc;
+      }
+    }
+  }
+  double2* M = p.seg_M + ((size_t)job * 4) * 32 + lane;      // [job][component][lane]
+  M[0] = make_double2(ar_, ai_);     // M11: P_s1   from (1, 0)
+  M[32] = make_double2(cr_, ci_);    // M12: P_s1   from (0, 1)
+  M[64] = make_double2(br_, bi_);    // M21: P_s1-1 from (1, 0)
+  M[96] = make_double2(dr_, di_);    // M22
+}
+
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 8)
+scalar_contour_segB_kernel(const ScalarLaunch p, const int n_warps) {
+  const int lane = threadIdx.x & 31;
+  const int ord = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
+  if (ord >= n_warps) return;
+  const ContourTask t = contour_task(p, ord, lane);
+  double qr = 1.0, qi = 0.0;                                                   // P_0
+  double pr = t.z.re - __ldg(t.U + t.i0) - t.sig_first.re, pi_ = t.z.im - t.sig_first.im;   // P_1
+  const double2* M = p.seg_M + ((size_t)ord * p.seg_S * 4) * 32 + lane;
+  double2* v = p.seg_v + ((size_t)ord * p.seg_S * 2) * 32 + lane;
+  for (int m = 0; m < p.seg_S; ++m, M += 4 * 32, v += 2 * 32) {
+    v[0] = make_double2(pr, pi_);                 // state at the start of segment m: P_s0, P_{s0-1}
+    v[32] = make_double2(qr, qi);
+    const double2 m11 = M[0], m12 = M[32], m21 = M[64], m22 = M[96];
+    const double nr = fma(m11.x, pr, fma(-m11.y, pi_, fma(m12.x, qr, -m12.y * qi)));
+    const double ni = fma(m11.x, pi_, fma(m11.y, pr, fma(m12.x, qi, m12.y * qr)));
+    const double or_ = fma(m21.x, pr, fma(-m21.y, pi_, fma(m22.x, qr, -m22.y * qi)));
+    const double oi = fma(m21.x, pi_, fma(m21.y, pr, fma(m22.x, qi, m22.y * qr)));
+    pr = nr; pi_ = ni; qr = or_; qi = oi;
+    const double mm = fma(pr, pr, pi_ * pi_);
+    const unsigned ex = (unsigned)(__double2hiint(mm) >> 20) - 623u;
+    if (ex > 800u && mm > 0.0) {
+      const double sc = (ex < 0x80000000u) ? 0x1p-200 : 0x1p200;
+      pr *= sc; pi_ *= sc; qr *= sc; qi *= sc;
+    }
+  }
+}
+
+__global__ void __launch_bounds__(128, 8) scalar_contour_segC_kernel(const ScalarLaunch p, const int n_warps) {
+  const int lane = threadIdx.x & 31;
+  const long long job = (long long)blockIdx.x * 4 + (threadIdx.x >> 5);
+  const int ord = (int)(job / p.seg_S), m = (int)(job - (long long)ord * p.seg_S);
+  if (ord >= n_warps) return;
+  const ContourTask t = contour_task(p, ord, lane);
+  int s0, s1;
+  seg_range(p, m, s0, s1);
+  if (m == 0) t.hist[(size_t)t.i0 * 32] = make_double2(t.sig_first.re, t.sig_first.im);   // the lead plays ring "-1"
+  const double2* v = p.seg_v + ((size_t)job * 2) * 32 + lane;
+  const double2 P = v[0], Q = v[32];
+  double pr = P.x, pi_ = P.y, qr = Q.x, qi = Q.y;
+  contour_steps(t, s0, s1, pr, pi_, qr, qi);
 }
 
 // Contour combine: G_(i,i) = 1 / (alpha_i - x_i - y_i) (Alg.1 step 1) and the first term
@@ -435,7 +543,15 @@ cudaError_t launch_scalar_sweep(const ScalarLaunch& p, cudaStream_t s) {
     if (n_c & 1) return cudaErrorInvalidValue;             // batches never split a contour pair
     if ((e = cudaEventRecord(p.ev_fork, s)) != cudaSuccess) return e;
     if ((e = cudaStreamWaitEvent(p.side, p.ev_fork, 0)) != cudaSuccess) return e;
-    scalar_contour_kernel<<<(n_c + kWarpsPerBlock - 1) / kWarpsPerBlock, kWarpsPerBlock * 32, 0, p.side>>>(p, n_c);
+    if (p.seg_M) {                                          // parallel in N (long channels)
+      const long long jobs = (long long)n_c * p.seg_S;
+      const unsigned blocks = (unsigned)((jobs + 3) / 4);
+      scalar_contour_segA_kernel<<<blocks, 128, 0, p.side>>>(p, n_c);
+      scalar_contour_segB_kernel<<<(n_c + kWarpsPerBlock - 1) / kWarpsPerBlock, kWarpsPerBlock * 32, 0, p.side>>>(p, n_c);
+      scalar_contour_segC_kernel<<<blocks, 128, 0, p.side>>>(p, n_c);
+    } else {
+      scalar_contour_kernel<<<(n_c + kWarpsPerBlock - 1) / kWarpsPerBlock, kWarpsPerBlock * 32, 0, p.side>>>(p, n_c);
+    }
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     for (int pair0 = 0; pair0 < n_c / 2; pair0 += 65535) {   // grid.y is limited to 65535
       dim3 grid((p.N + 127) / 128, std::min(65535, n_c / 2 - pair0));

@@ -294,3 +294,43 @@ def test_integrand_probe_and_peak_vs_definition(cfg, kw, ring):
     with pytest.raises(Exception):
         h.negf_integrand_peak(I, kp, Ep)
     h.negf_destroy()
+
+
+def _charge_with_env(wl, env):
+    import os
+    import torch
+    from paper_2407_14633_b200 import Negf
+    old = {k: os.environ.get(k) for k in env}
+    os.environ.update(env)
+    try:
+        h = Negf.from_workload(wl)
+    finally:
+        for k, v in old.items():
+            if v is None:
+                os.environ.pop(k, None)
+            else:
+                os.environ[k] = v
+    n = torch.empty((wl.C, wl.N), dtype=torch.float64, device="cuda")
+    h.negf_set_potential(torch.tensor(wl.phi, dtype=torch.float64, device="cuda"))
+    h.negf_charge(n)
+    h.negf_sync()
+    plan = h.negf_get_plan()
+    h.negf_destroy()
+    return n.cpu().numpy(), plan
+
+
+@pytest.mark.parametrize("N,seg_len", [(300, 7), (257, 256), (64, 1), (2, 5), (3, 1), (1000, 33)])
+def test_parallel_in_N_contour_path_vs_definition_and_serial(N, seg_len):
+    """the segmented (parallel-in-N) contour half-sweeps -- segment transfer products, serial
+    pass over the segment starts, parallel re-run of every segment -- against the dense definition
+    (N <= 300) and against the serial pass of the same library: several segments, a ragged last segment,
+    one-step segments, N = 2 and 3, both contour directions, config 2's mix of real-axis and contour tasks."""
+    wl = wlmod.table2(N=N) if N != 1000 else wlmod.make_config(2, N=1000, K_neq=64, K_eq=24)
+    n_seg, plan_seg = _charge_with_env(wl, {"NEGF_SEG_MIN_RINGS": "2", "NEGF_SEG_LEN": str(seg_len)})
+    n_ser, plan_ser = _charge_with_env(wl, {"NEGF_SEG_MIN_RINGS": "1000000000"})
+    if N >= 3:
+        assert plan_seg["kernel_launches"] == plan_ser["kernel_launches"] + 2      # 3 contour kernels instead of 1
+    assert_parity(n_seg, n_ser, f"segmented vs serial contour pass, N={N}", rtol=1e-12)
+    if N <= 300:
+        n_ref, _ = od.charge_and_transmission(wl)
+        assert_parity(n_seg, n_ref, f"segmented contour pass vs dense definition, N={N}")
