@@ -96,6 +96,26 @@ def test_forced_column_search_matches():
         assert_parity(T, T_ref, f"{w.name} forced-search T(E)")
 
 
+def test_integrand_probe_generic_block_sizes():
+    """SURVEY 8(f)-2 on the SIMT way back of the generic block sizes (n != 17): integrand at a probe ring
+    and its peak against the dense definition, random non-symmetric complex blocks."""
+    import torch
+    from paper_2407_14633_b200 import Negf
+    for n, ring in ((5, 3), (3, 0), (8, 6)):
+        wl = _random_block_workload(n, N=7, K_neq=12, K_eq=2, seed=90 + n, C=2)
+        I_ref = od.integrand_dense(wl, ring)
+        h = Negf.from_workload(wl)
+        h.negf_set_potential(torch.tensor(wl.phi, dtype=torch.float64, device="cuda"))
+        h.negf_set_probe(ring)
+        I = torch.empty((wl.C, wl.K_neq), dtype=torch.float64, device="cuda")
+        kp = torch.empty(wl.C, dtype=torch.int32, device="cuda")
+        h.negf_integrand_peak(I, kp, None)
+        h.negf_sync()
+        assert_parity(I.cpu().numpy(), I_ref, f"random n={n} integrand at ring {ring}")
+        assert np.array_equal(kp.cpu().numpy(), np.argmax(I_ref, axis=1))
+        h.negf_destroy()
+
+
 def test_config4_shrunk_multi_channel():
     wl = wlmod.make_config(4, C=3, N=14, K_neq=19, K_eq=5)
     n_ref, T_ref = od.charge_and_transmission(wl)
