@@ -59,3 +59,29 @@ def test_reference_arm_runs_on_rank0_only():
     line = lines[0]
     assert line["impl"] == "reference" and line["n_gpus"] == 2 and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_poisson_stand_in_as_one_sparse_matrix():
+    """bench.py applies the Poisson stand-in of config 5 (harness code) as one SpMV; the CSR matrix must
+    be the very map of workloads.PoissonStandIn.apply_K, for one and for several channels."""
+    import numpy as np
+    import torch
+    sys.path.insert(0, ROOT)
+    import bench
+    import workloads as wlmod
+    rng = np.random.default_rng(3)
+    for C, N in ((1, 23), (4, 17)):
+        p = wlmod.PoissonStandIn(kappa=0.2, r=rng.uniform(0.5, 1.0, (max(C - 1, 0), N)), n0=17.0)
+        rowptr, cols, vals = p.as_csr(C, N)
+        assert rowptr[-1] == len(cols) == len(vals) and np.all(np.diff(rowptr) >= 4)
+        # diagonally dominant, off-diagonal row sum <= 0.9 kappa (BASELINE.json configs[4])
+        dense = np.zeros((C * N, C * N))
+        for i in range(C * N):
+            dense[i, cols[rowptr[i]:rowptr[i + 1]]] = vals[rowptr[i]:rowptr[i + 1]]
+        assert np.allclose(np.diag(dense), 0.2) and np.all(dense.sum(1) - 0.2 <= 0.9 * 0.2 + 1e-15)
+        q = rng.normal(size=(C, N))
+        assert np.max(np.abs(dense @ q.ravel() - p.apply_K(q.copy()).ravel())) < 1e-15
+        pd = bench.PoissonOnDevice(p, C, N, "cpu")
+        phi_ext = torch.tensor(rng.normal(size=(C, N)))
+        n = torch.tensor(q + 17.0)
+        assert np.max(np.abs(pd.phi_out(phi_ext, n).numpy() - p.phi_out(phi_ext.numpy(), n.numpy()))) < 1e-15
