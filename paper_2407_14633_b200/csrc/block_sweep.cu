@@ -177,7 +177,11 @@ __global__ void __launch_bounds__(Geo2<NB>::THREADS, (NB >= 16 ? 4 : 1)) block_s
       asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(dst + 2 * j), "d"(row[2 * j].x),
                    "d"(row[2 * j].y), "d"(row[2 * j + 1].x), "d"(row[2 * j + 1].y)
                    : "memory");
-    dst[16] = row[NB - 1];
+    // the 17th element together with the padding element 17: a full 32-byte sector, so that L2 does not
+    // have to fetch the other half from DRAM (the 16-byte tail store cost 9.2 GB of reads per config-4 launch)
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(dst + 16), "d"(row[NB - 1].x), "d"(row[NB - 1].y),
+                 "d"(0.0), "d"(0.0)
+                 : "memory");
   };
   auto store_history = [&](const c64 (&y)[2][NB], int s) {
     if (!live) return;
