@@ -271,12 +271,13 @@ def sancho_rubio_line(wl, stats, plan, steps, dfma_peak):
         return None
     passes = plan.get("sr_passes_total", 0)
     m = 2 * wl.n
-    per_launch_ms = ms / launches
+    per_launch_ms = ms / steps                      # per negf_set_potential (one or, in the overlap plan, two launches)
     flop_alg = 56.0 * m ** 3 * passes
     flop_exec = 128.0 * wl.n ** 3 * passes
     tf_alg = flop_alg / (per_launch_ms * 1e-3) / 1e12
     tf_exec = flop_exec / (per_launch_ms * 1e-3) / 1e12
     return {"kernel": "sancho_rubio", "bound": "alu", "kernel_ms_per_launch": per_launch_ms,
+            "launches_per_set_potential": launches / steps,
             "passes_total": int(passes), "tasks": int(wl.C * (wl.K_eq + wl.K_neq) * 2),
             "max_passes": int(plan.get("max_sr_iterations", 0)),
             "algorithmic_flop_per_launch": flop_alg, "achieved": tf_alg, "unit": "TFLOP/s",

@@ -4,6 +4,7 @@
 // chain (sancho_rubio.cu header), computed once at creation.
 #include <algorithm>
 #include <complex>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -41,6 +42,14 @@ struct BlockPath {
   double2* hist;
   double* partial;
   double* scratch;
+  // Overlap plan (C = 1, one launch, the real-axis CTAs alone fit one wave but all CTAs do not -- config 3):
+  // negf_set_potential runs the self-energies of the contour energies first and then starts the contour
+  // half-sweeps + combine on a side stream, beside the self-energies of the real-axis energies; negf_charge
+  // launches the real-axis CTAs only and joins.  Without it the few contour CTAs cost a second forward wave.
+  bool overlap, contour_started;
+  cudaStream_t side;
+  cudaEvent_t ev_fork, ev_join;
+  const double* U_last;   // potential the contour sweep was started for
   int* flags;       // [0] max SR iterations, [1] non-convergence flag
   unsigned long long* counters;   // [0] Sancho-Rubio passes of the last set_potential, summed over all tasks
   int last_max_iters;
@@ -87,6 +96,9 @@ void block_path_destroy(BlockPath* bp) {
   cudaFree(bp->csr_rowptr); cudaFree(bp->csr_col); cudaFree(bp->csr_val); cudaFree(bp->csr_diag);
   cudaFree(bp->lead_mats); cudaFree(bp->table); cudaFree(bp->hist);
   cudaFree(bp->partial); cudaFree(bp->scratch); cudaFree(bp->flags); cudaFree(bp->counters);
+  if (bp->side) { cudaStreamSynchronize(bp->side); cudaStreamDestroy(bp->side); }
+  if (bp->ev_fork) cudaEventDestroy(bp->ev_fork);
+  if (bp->ev_join) cudaEventDestroy(bp->ev_join);
   delete bp;
 }
 
@@ -244,6 +256,25 @@ negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, c
   bp->slots = (int)slots;
   bp->hist_bytes = bp->slot_bytes * slots;
   bp->n_launches = (int)((bp->total_cta + slots - 1) / slots);
+  {
+    const char* force = getenv("NEGF_FORCE_OVERLAP");   // test hook: "1" forces the plan on small devices, "0" forbids it
+    const bool possible = bp->C == 1 && bp->n_launches == 1 && bp->n_eq_cta > 0 && bp->total_cta > bp->n_eq_cta;
+    const bool pays = bp->total_cta > bp->wave && bp->total_cta - bp->n_eq_cta <= bp->wave;
+    bp->overlap = possible && (force ? force[0] == '1' : pays);
+  }
+  if (bp->overlap) {
+    // highest priority: when the contour CTAs and the second Sancho-Rubio launch become ready together, the
+    // few contour CTAs must be placed first (a Sancho-Rubio CTA takes a whole SM's registers)
+    int prio_lo = 0, prio_hi = 0;
+    cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+    chk(cudaStreamCreateWithPriority(&bp->side, cudaStreamNonBlocking, prio_hi));
+    chk(cudaEventCreateWithFlags(&bp->ev_fork, cudaEventDisableTiming));
+    chk(cudaEventCreateWithFlags(&bp->ev_join, cudaEventDisableTiming));
+    if (e != cudaSuccess) {
+      set_error("negf_create: cannot create the side stream: %s", cudaGetErrorString(e));
+      return fail(NEGF_ECUDA);
+    }
+  }
   e = cudaMalloc((void**)&bp->hist, (size_t)bp->hist_bytes);
   if (e != cudaSuccess) {
     set_error("negf_create: cannot allocate %lld bytes of recursion history: %s", (long long)bp->hist_bytes,
@@ -251,6 +282,37 @@ negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, c
     return fail(NEGF_ENOMEM);
   }
   *out = bp;
+  return NEGF_OK;
+}
+
+namespace {
+
+blk::SweepLaunch sweep_launch(const BlockPath* bp, const double* U_dev, double* T_res, int probe_ring, double* probe) {
+  blk::SweepLaunch p;
+  p.C = bp->C; p.N = bp->N; p.K_eq = bp->K_eq; p.K_neq = bp->K_neq;
+  p.geq = bp->geq; p.gneq = bp->gneq; p.n_eq_cta = bp->n_eq_cta;
+  p.U = U_dev; p.z_eq = bp->z_eq; p.w_eq = bp->w_eq; p.z_neq = bp->z_neq; p.w_neq = bp->w_neq;
+  p.table = bp->table;
+  p.mu_s = bp->mu_s; p.mu_d = bp->mu_d; p.kT = bp->kT; p.deg = bp->deg; p.theta2 = bp->theta2;
+  p.hist = bp->hist; p.partial = bp->partial; p.T = T_res;
+  p.probe_ring = probe_ring; p.probe = probe;
+  p.csr.rowptr = bp->csr_rowptr; p.csr.col = bp->csr_col; p.csr.val = bp->csr_val;
+  p.csr.nnz_cap = bp->nnz_cap;
+  p.csr.diag = bp->csr_diag; p.csr.diag_mask = bp->diag_mask;
+  p.cta_begin = 0;
+  p.n_cta = 0;
+  return p;
+}
+
+}  // namespace
+
+negf_status block_path_before_potential(BlockPath* bp, cudaStream_t s) {
+  // Overlap plan: a contour sweep started for the previous potential and never joined (two
+  // negf_set_potential calls in a row) still reads U and the table: the stream waits for it first.
+  if (bp->overlap && bp->contour_started) {
+    NEGF_CUDA_TRY(cudaStreamWaitEvent(s, bp->ev_join, 0));
+    bp->contour_started = false;
+  }
   return NEGF_OK;
 }
 
@@ -265,8 +327,40 @@ negf_status block_path_self_energy(BlockPath* bp, const double* U_dev, cudaStrea
   // [0] = largest iteration count of THIS call; [1] = non-convergence flag, sticky until block_path_check
   // has reported it (a Broyden loop that never syncs in between must not lose it)
   NEGF_CUDA_TRY(cudaMemsetAsync(bp->flags, 0, sizeof(int), s));
+  const long long n_task = (long long)bp->C * ((long long)bp->K_eq + bp->K_neq) * 2;
+  if (!bp->overlap) {
+    p.task_begin = 0;
+    p.task_end = n_task;
+    hook.begin(hook.ctx, 0);
+    cudaError_t e = blk::launch_sancho_rubio(bp->n, p, s);
+    hook.end(hook.ctx);
+    NEGF_CUDA_TRY(e);
+    return NEGF_OK;
+  }
+  // overlap plan (C = 1: the contour energies are the first 2 K_eq tasks): self-energies of the contour
+  // energies, then the contour half-sweeps + combine on the side stream beside the rest of the self-energies
+  p.task_begin = 0;
+  p.task_end = 2LL * bp->K_eq;
   hook.begin(hook.ctx, 0);
   cudaError_t e = blk::launch_sancho_rubio(bp->n, p, s);
+  hook.end(hook.ctx);
+  NEGF_CUDA_TRY(e);
+  NEGF_CUDA_TRY(cudaEventRecord(bp->ev_fork, s));
+  NEGF_CUDA_TRY(cudaStreamWaitEvent(bp->side, bp->ev_fork, 0));
+  {
+    blk::SweepLaunch q = sweep_launch(bp, U_dev, nullptr, -1, nullptr);
+    q.cta_begin = 0;
+    q.n_cta = (int)bp->n_eq_cta;
+    NEGF_CUDA_TRY(blk::launch_block_sweep(bp->n, q, bp->side));
+    NEGF_CUDA_TRY(blk::launch_block_combine(bp->n, q, 0, (int)(bp->n_eq_cta / 2), bp->side));
+  }
+  NEGF_CUDA_TRY(cudaEventRecord(bp->ev_join, bp->side));
+  bp->contour_started = true;
+  bp->U_last = U_dev;
+  p.task_begin = 2LL * bp->K_eq;
+  p.task_end = n_task;
+  hook.begin(hook.ctx, 0);
+  e = blk::launch_sancho_rubio(bp->n, p, s);
   hook.end(hook.ctx);
   NEGF_CUDA_TRY(e);
   return NEGF_OK;
@@ -274,30 +368,38 @@ negf_status block_path_self_energy(BlockPath* bp, const double* U_dev, cudaStrea
 
 negf_status block_path_run(BlockPath* bp, const double* U_dev, double* n_res, double* T_res, int probe_ring,
                            double* probe, cudaStream_t s, ProfHook hook) {
-  blk::SweepLaunch p;
-  p.C = bp->C; p.N = bp->N; p.K_eq = bp->K_eq; p.K_neq = bp->K_neq;
-  p.geq = bp->geq; p.gneq = bp->gneq; p.n_eq_cta = bp->n_eq_cta;
-  p.U = U_dev; p.z_eq = bp->z_eq; p.w_eq = bp->w_eq; p.z_neq = bp->z_neq; p.w_neq = bp->w_neq;
-  p.table = bp->table;
-  p.mu_s = bp->mu_s; p.mu_d = bp->mu_d; p.kT = bp->kT; p.deg = bp->deg; p.theta2 = bp->theta2;
-  p.hist = bp->hist; p.partial = bp->partial; p.T = T_res;
-  p.probe_ring = probe_ring; p.probe = probe;
-  p.csr.rowptr = bp->csr_rowptr; p.csr.col = bp->csr_col; p.csr.val = bp->csr_val;
-  p.csr.nnz_cap = bp->nnz_cap;
-  p.csr.diag = bp->csr_diag; p.csr.diag_mask = bp->diag_mask;
-  for (long long begin = 0; begin < bp->total_cta; begin += bp->slots) {
-    p.cta_begin = begin;
-    p.n_cta = (int)std::min<long long>(bp->slots, bp->total_cta - begin);
+  blk::SweepLaunch p = sweep_launch(bp, U_dev, T_res, probe_ring, probe);
+  if (bp->overlap && bp->contour_started && bp->U_last == U_dev) {
+    // the contour CTAs run (or ran) on the side stream in the slots [0, n_eq_cta): the real-axis CTAs go to
+    // the slots after them, in one wave
+    p.cta_begin = bp->n_eq_cta;
+    p.n_cta = (int)(bp->total_cta - bp->n_eq_cta);
+    p.hist = bp->hist + (size_t)bp->n_eq_cta * bp->N * blk::block_step_elems(bp->n);
     hook.begin(hook.ctx, 1);
     cudaError_t e = blk::launch_block_sweep(bp->n, p, s);
     hook.end(hook.ctx);
     NEGF_CUDA_TRY(e);
-    const long long eq_end = std::min<long long>(begin + p.n_cta, bp->n_eq_cta);
-    if (eq_end > begin) {
-      hook.begin(hook.ctx, 3);
-      e = blk::launch_block_combine(bp->n, p, begin, (int)((eq_end - begin) / 2), s);
+    NEGF_CUDA_TRY(cudaStreamWaitEvent(s, bp->ev_join, 0));
+    bp->contour_started = false;
+  } else {
+    if (bp->overlap && bp->contour_started) {          // started for another potential buffer: join, redo below
+      NEGF_CUDA_TRY(cudaStreamWaitEvent(s, bp->ev_join, 0));
+      bp->contour_started = false;
+    }
+    for (long long begin = 0; begin < bp->total_cta; begin += bp->slots) {
+      p.cta_begin = begin;
+      p.n_cta = (int)std::min<long long>(bp->slots, bp->total_cta - begin);
+      hook.begin(hook.ctx, 1);
+      cudaError_t e = blk::launch_block_sweep(bp->n, p, s);
       hook.end(hook.ctx);
       NEGF_CUDA_TRY(e);
+      const long long eq_end = std::min<long long>(begin + p.n_cta, bp->n_eq_cta);
+      if (eq_end > begin) {
+        hook.begin(hook.ctx, 3);
+        e = blk::launch_block_combine(bp->n, p, begin, (int)((eq_end - begin) / 2), s);
+        hook.end(hook.ctx);
+        NEGF_CUDA_TRY(e);
+      }
     }
   }
   hook.begin(hook.ctx, 2);
@@ -346,7 +448,8 @@ void block_path_plan(BlockPath* bp, negf_plan_info* out) {
     sweeps += (bp->n == 17 && b + bp->slots > bp->n_eq_cta) ? 2 : 1;
     if (b < bp->n_eq_cta) ++combines;
   }
-  out->kernel_launches = 1 + 1 + sweeps + combines + 2;
+  // overlap plan: two Sancho-Rubio launches and a contour sweep launch of its own
+  out->kernel_launches = 1 + 1 + sweeps + combines + 2 + (bp->overlap ? 2 : 0);
 }
 
 }  // namespace negf

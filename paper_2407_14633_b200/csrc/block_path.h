@@ -22,6 +22,8 @@ struct ProfHook {                 // optional per-kernel timing callbacks (kinds
 
 negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, const double2* w_eq_dev,
                               const double2* z_neq_dev, const double* w_neq_dev, BlockPath** out);
+// to be called before U is overwritten by a new potential (joins a contour sweep still in flight)
+negf_status block_path_before_potential(BlockPath* bp, cudaStream_t s);
 negf_status block_path_self_energy(BlockPath* bp, const double* U_dev, cudaStream_t s, ProfHook hook);
 negf_status block_path_run(BlockPath* bp, const double* U_dev, double* n_res, double* T_res, int probe_ring,
                            double* probe, cudaStream_t s, ProfHook hook);
@@ -60,6 +62,7 @@ struct SrLaunch {
   int* max_iters;             // device scalar, atomicMax
   int* noconv_flag;           // device scalar
   unsigned long long* iters_total;   // device scalar: decimation passes summed over all tasks
+  long long task_begin, task_end;    // this launch covers the tasks [task_begin, task_end) of the C * K_all * 2
 };
 cudaError_t launch_sancho_rubio(int nb, const SrLaunch& p, cudaStream_t s);
 

@@ -385,6 +385,10 @@ extern "C" negf_status negf_create(const negf_config* cfg, void* cuda_stream, ne
 
 extern "C" negf_status negf_set_potential(negf_handle* h, const double* phi_dev) {
   if (!h || !phi_dev) { set_error("negf_set_potential: null argument"); return NEGF_EINVAL; }
+  if (!h->scalar) {
+    negf_status st = block_path_before_potential(h->block, h->stream);
+    if (st != NEGF_OK) return st;
+  }
   {
     ProfScope ps(h, K_MISC);
     NEGF_CUDA_TRY(launch_negate(phi_dev, h->U, (int64_t)h->C * h->N, h->stream));   // U = -e phi

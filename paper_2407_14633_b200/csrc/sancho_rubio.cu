@@ -98,8 +98,8 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
   c64* other = h == 0 ? Xb : Yb;
 
   const int K_all = p.K_eq + p.K_neq;
-  const long long n_task = (long long)p.C * K_all * 2;
-  long long task = (long long)blockIdx.x * G2::TPC + t;
+  const long long n_task = p.task_end;
+  long long task = p.task_begin + (long long)blockIdx.x * G2::TPC + t;
   const bool active = live && task < n_task;
   if (task >= n_task) task = n_task - 1;
   const int lead = (int)(task & 1);
@@ -432,7 +432,8 @@ static cudaError_t launch_sr_t(const SrLaunch& p, cudaStream_t s) {
   cudaError_t e = cudaFuncSetAttribute(sancho_rubio_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)smem);
   if (e != cudaSuccess) return e;
-  const long long n_task = (long long)p.C * (p.K_eq + p.K_neq) * 2;
+  const long long n_task = p.task_end - p.task_begin;
+  if (n_task <= 0) return cudaSuccess;
   const int blocks = (int)((n_task + G2::TPC - 1) / G2::TPC);
   sancho_rubio_kernel<NB><<<blocks, G2::THREADS, smem, s>>>(p);
   return cudaGetLastError();

@@ -146,6 +146,47 @@ def test_workspace_tiling_gives_identical_results():
     assert np.array_equal(n1, n2) and np.array_equal(T1, T2)
 
 
+def test_overlap_plan_gives_identical_results():
+    """The overlap plan of config 3 (contour half-sweeps on a side stream beside the self-energies of the
+    real-axis energies, real-axis CTAs in their own launch) forced on a small device: same results as the
+    single-launch plan (to rounding: the two Sancho-Rubio launches group the tasks into CTAs differently, and
+    a task polishes as long as its CTA-mates do), also when negf_set_potential is called twice before
+    negf_charge and when the sweep is re-run for a probe."""
+    import os
+    import torch
+    from paper_2407_14633_b200 import Negf
+    wl = wlmod.make_config(3, N=14, K_neq=30, K_eq=9)
+    out = {}
+    for mode in ("0", "1"):
+        os.environ["NEGF_FORCE_OVERLAP"] = mode
+        try:
+            h = Negf.from_workload(wl)
+        finally:
+            del os.environ["NEGF_FORCE_OVERLAP"]
+        phi = torch.tensor(wl.phi, dtype=torch.float64, device="cuda")
+        n = torch.empty((wl.C, wl.N), dtype=torch.float64, device="cuda")
+        T = torch.empty((wl.C, wl.K_neq), dtype=torch.float64, device="cuda")
+        h.negf_set_potential(phi * 0.5)            # overwritten before any charge: the stale contour sweep must be joined
+        h.negf_set_potential(phi)
+        h.negf_charge(n)
+        h.negf_transmission(T)
+        h.negf_sync()
+        a = (n.cpu().numpy().copy(), T.cpu().numpy().copy())
+        h.negf_set_probe(3)                         # re-runs the sweep for the same potential
+        h.negf_charge(n)
+        h.negf_sync()
+        assert np.array_equal(a[0], n.cpu().numpy())
+        plan = h.negf_get_plan()
+        h.negf_destroy()
+        out[mode] = a + (plan["kernel_launches"],)
+    assert out["1"][2] == out["0"][2] + 2
+    assert_parity(out["1"][0], out["0"][0], "overlap vs single-launch charge", rtol=1e-12)
+    assert_parity(out["1"][1], out["0"][1], "overlap vs single-launch T(E)", rtol=1e-10)
+    n_ref, T_ref = od.charge_and_transmission(wl)
+    assert_parity(out["1"][0], n_ref, "overlap plan charge")
+    assert_parity(out["1"][1], T_ref, "overlap plan T(E)")
+
+
 def test_config3_full_length_sampled_vs_paper_recursion():
     """Full device length (N = 1000, the bench launch geometry: 256-thread CTAs, 15 tasks each) on a
     sample of configs[2]'s energies against tier O3."""
