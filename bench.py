@@ -473,7 +473,7 @@ def measure(config, steps, warmup, world, dev, stream, peaks, e2e_steps=None, sa
 
 
 # timed steps / warm-ups of the per_config legs (bounded so that the default run finishes within minutes)
-PER_CONFIG_STEPS = {1: (50, 3), 2: (50, 3), 3: (5, 3), 4: (3, 3), 5: (2, 3), 6: (3, 3)}
+PER_CONFIG_STEPS = {1: (50, 3), 2: (50, 3), 3: (5, 3), 4: (3, 3), 5: (2, 1), 6: (3, 3)}
 
 
 def run_ours(args):
