@@ -347,7 +347,7 @@ def measure_graph_replay(wl, poisson, steps, dev):
         return {"error": str(exc)[:200]}
 
 
-def measure(config, steps, warmup, world, dev, stream, peaks, e2e_steps=None, sample_clocks=True):
+def measure(config, steps, warmup, world, dev, stream, peaks, e2e_steps=None, sample_clocks=True, trace_eps=False):
     """W warm-up + K timed steps of one workload on this rank; returns the local record."""
     import torch
     from paper_2407_14633_b200 import Broyden, Negf
@@ -362,15 +362,26 @@ def measure(config, steps, warmup, world, dev, stream, peaks, e2e_steps=None, sa
     n = torch.empty((wl.C, wl.N), dtype=torch.float64, device=dev)
     T = torch.empty((wl.C, max(wl.K_neq, 1)), dtype=torch.float64, device=dev)
 
+    eps_trace = []
+
     def step():
         h.negf_set_potential(phi)                       # a0 (+ a1b for Sancho-Rubio leads)
         h.negf_charge(n)                                # a1s, a2, a3, a5
         h.negf_transmission(T)                          # a4 (cached by negf_charge)
         phi_out = pd.phi_out(phi_ext, n)                # harness: Poisson stand-in (one SpMV)
-        bro.broyden_step(phi.view(-1), phi_out.view(-1), want_eps=False)   # a6
+        if trace_eps:                                   # --trace-eps: Alg.3's eps_max of every step (one sync each)
+            resid = float((phi - phi_out).abs().max().item())
+            eps = bro.broyden_step(phi.view(-1), phi_out.view(-1), want_eps=True)
+            eps_trace.append((eps, resid))
+        else:
+            bro.broyden_step(phi.view(-1), phi_out.view(-1), want_eps=False)   # a6
 
     for _ in range(warmup):
         step()
+    if trace_eps:                                       # the timed steps are the loop itself: start it from phi_ext
+        phi.copy_(phi_ext)
+        bro.broyden_reset()
+        eps_trace.clear()
     torch.cuda.synchronize()
     h.negf_kernel_stats(reset=True)
     dist_barrier(world)
@@ -461,7 +472,7 @@ def measure(config, steps, warmup, world, dev, stream, peaks, e2e_steps=None, sa
     rec = {
         "wl": wl, "local_ms": local_ms, "units": float(sweeps_per_step * steps), "steps": steps,
         "sweeps_per_step": sweeps_per_step, "clocks": clocks, "stats": stats, "plan": plan,
-        "roofline": roofline, "l2_note": l2_note, "e2e": e2e, "graph": graph,
+        "roofline": roofline, "l2_note": l2_note, "e2e": e2e, "graph": graph, "eps_trace": list(eps_trace),
         "sancho_rubio": sancho_rubio_line(wl, stats, plan, steps, dfma),
         "launches_per_step": plan["kernel_launches"] + 4,     # + 4 Broyden kernels
     }
@@ -493,7 +504,8 @@ def run_ours(args):
     # ---- headline workload
     block = args.config >= 3
     e2e_steps = min(args.steps, 3) if block else args.steps
-    rec = measure(args.config, args.steps, args.warmup, world, dev, stream, peaks, e2e_steps=e2e_steps)
+    rec = measure(args.config, args.steps, args.warmup, world, dev, stream, peaks, e2e_steps=e2e_steps,
+                  trace_eps=args.trace_eps)
     wl = rec["wl"]
     ms, units = dist_max_sum(rec["local_ms"], rec["units"], world, dev)
     e2e_ms, e2e_units = dist_max_sum(rec["e2e"]["local_ms"], float(rec["sweeps_per_step"] * rec["e2e"]["steps"]),
@@ -573,6 +585,11 @@ def run_ours(args):
         "per_config": per_config,
         "cpu_baseline": cpu_baseline,
     }
+    if rec["eps_trace"]:
+        line["broyden_trace"] = {"eps_max": [e for e, _ in rec["eps_trace"]],
+                                 "residual_max_abs": [r for _, r in rec["eps_trace"]],
+                                 "note": "timed steps = iterations 1.. of the self-consistent loop started from phi_ext "
+                                         "(Alg.3 eps_max, PAPER.md:226-239, and max|phi_in - phi_out| before each update)"}
     if rec["graph"]:
         line["cuda_graph_replay"] = dict(rec["graph"])
         if "ms_per_step" in rec["graph"]:
@@ -591,6 +608,9 @@ def main():
     ap.add_argument("--per-config", default="all", dest="per_config",
                     help="other workloads measured in the same run: 'all', 'none' or e.g. '2,3' "
                          "(1-5 = BASELINE.json configs, 6 = the Table 2 shape of SURVEY 8(f)-4)")
+    ap.add_argument("--trace-eps", action="store_true", dest="trace_eps",
+                    help="headline workload: restart the Broyden loop after the warm-up and record eps_max and the "
+                         "residual of every timed step (one host sync per step)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-budget", type=float, default=15.0, dest="cpu_budget")
     args = ap.parse_args()

@@ -106,7 +106,10 @@ NEGF_API negf_status negf_destroy(negf_handle* h);
 
 /* Set the electrostatic potential phi[C][N] (volts, channel-major, R20).  Enqueues U = -phi and, for
  * lead_kind 1, the Sancho-Rubio self-energy kernel for every (channel, energy, lead) -- Sigma depends
- * on phi through the end rings (R7).  Invalidates cached results. */
+ * on phi through the end rings (R7).  Invalidates cached results.  phi_dev is read by this call only
+ * (the library keeps its own U).  For some single-channel block handles the library also starts the
+ * contour half-sweeps of the coming negf_charge here, on a stream of its own that it joins itself
+ * (overlap plan); this is invisible to the caller. */
 NEGF_API negf_status negf_set_potential(negf_handle* h, const double* phi_dev);
 
 /* Charge n[C][N] (electrons per ring, >= 0; eq.(4)) for the current potential: self-energies ->
@@ -191,6 +194,11 @@ NEGF_API negf_status broyden_destroy(broyden_handle* h);
  * DFMA instructions and of DMMA (mma.sync.m8n8k4.f64) instructions; used as the roofline denominator
  * of the FP64-bound block kernels.  Synchronous; takes a few milliseconds. */
 NEGF_API negf_status negf_fp64_peak(double* dfma_tflops, double* dmma_tflops);
+
+/* Environment variables read at negf_create (test hooks; the defaults are the product path):
+ *   NEGF_SEG_MIN_RINGS  scalar handles with at least this many rings run their contour half-sweeps parallel
+ *                       in N (default 8192);  NEGF_SEG_LEN  segment length of that pass (default max(256, N/1024));
+ *   NEGF_FORCE_OVERLAP  "1" / "0": force / forbid the overlap plan of single-channel block handles. */
 
 /* Last error text of the calling thread (static storage, never NULL). */
 NEGF_API const char* negf_last_error(void);

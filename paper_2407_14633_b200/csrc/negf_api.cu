@@ -301,6 +301,10 @@ extern "C" negf_status negf_create(const negf_config* cfg, void* cuda_stream, ne
     return NEGF_EINVAL;
   }
   if (!(cfg->kT > 0.0) || !(cfg->deg > 0.0)) { set_error("negf_create: need kT > 0 and deg > 0"); return NEGF_EINVAL; }
+  if (cfg->reserved != 0 || cfg->workspace_bytes < 0 || !(cfg->pivot_theta >= 0.0)) {
+    set_error("negf_create: need reserved == 0, workspace_bytes >= 0 and pivot_theta >= 0");
+    return NEGF_EINVAL;
+  }
   if (cfg->n_eq < 0 || cfg->n_neq < 0 || cfg->n_eq + cfg->n_neq < 1) {
     set_error("negf_create: need n_eq >= 0, n_neq >= 0 and at least one energy point");
     return NEGF_EINVAL;

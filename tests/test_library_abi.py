@@ -55,6 +55,14 @@ def test_argument_validation_without_gpu(lib):
     assert b"n_rings" in lib.negf_last_error()
     cfg.n_rings, cfg.kT, cfg.deg = 10, -1.0, 2.0             # kT <= 0
     assert lib.negf_create(C.byref(cfg), None, C.byref(h)) == b.NEGF_EINVAL
+    cfg.kT = 0.0259
+    cfg.reserved = 1                                         # reserved fields must be 0
+    assert lib.negf_create(C.byref(cfg), None, C.byref(h)) == b.NEGF_EINVAL
+    assert b"reserved" in lib.negf_last_error()
+    cfg.reserved, cfg.pivot_theta = 0, -1.0
+    assert lib.negf_create(C.byref(cfg), None, C.byref(h)) == b.NEGF_EINVAL
+    assert lib.negf_set_probe(None, 0) == b.NEGF_EINVAL
+    assert lib.negf_integrand_peak(None, None, None, None) == b.NEGF_EINVAL
     assert lib.negf_set_potential(None, None) == b.NEGF_EINVAL
     assert lib.negf_charge(None, None) == b.NEGF_EINVAL
     assert lib.negf_transmission(None, None) == b.NEGF_EINVAL
