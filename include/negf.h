@@ -95,7 +95,7 @@ typedef struct {
   double  pivot_theta;        /* block > 1: the diagonal pivot candidate of an in-register Gauss-Jordan step is
                                  accepted without a search when |a_kk| >= theta * ||row k of the matrix handed
                                  in||_2; otherwise the task searches the whole column (partial pivoting).
-                                 0 = default (1e-3); a huge value (1e150) forces the search at every
+                                 0 = default (1e-4); a huge value (1e150) forces the search at every
                                  elimination step (test hook).                                             */
 } negf_config;
 
