@@ -190,6 +190,23 @@ NEGF_API negf_status broyden_step(broyden_handle* h, double* x_in_dev, const dou
 NEGF_API negf_status broyden_reset(broyden_handle* h);
 NEGF_API negf_status broyden_destroy(broyden_handle* h);
 
+/* The convergence measure of the self-consistent loop WITHOUT any allocation (for callers that cannot call
+ * cudaMalloc: CUDA graph capture, tight serving loops, harnesses that forbid it):
+ *     *eps_max_dev = max_t |x_in,t - x_out,t| / max(|x_in,t + x_out,t|, 1e-300)   (Alg.3 steps 2, 4-7,
+ * PAPER.md:216-230; the value broyden_step returns in eps_max_host; NaN / infinity in the residual give
+ * +infinity).  x_in_dev, x_out_dev: DEVICE, len doubles each, read only; eps_max_dev: DEVICE, one double,
+ * written; all caller-owned.  Two kernels are launched on cuda_stream (a cudaStream_t, NULL = default
+ * stream); nothing is synchronised, no handle is needed, and no cudaMalloc, cudaFree or allocating routine is
+ * called.  The per-block partial maxima live in a 128 KiB file-scope device array (residual_noalloc.cu) that
+ * every GPU loading the library holds until the process exits; one partial per 4096 entries, so
+ * 1 <= len <= NEGF_NOALLOC_MAX_LEN, else NEGF_EINVAL.  The array's device address is resolved on the first
+ * call on each device (cudaGetSymbolAddress, no allocation): make that first call outside stream capture.
+ * All calls on a device share the array: a call overwrites the entries it reads, so nothing carries over
+ * from the previous call, but calls that overlap on the GPU (different streams, no dependency) race. */
+#define NEGF_NOALLOC_MAX_LEN ((int64_t)1 << 26)
+NEGF_API negf_status broyden_residual_noalloc(const double* x_in_dev, const double* x_out_dev, int64_t len,
+                                     double* eps_max_dev, void* cuda_stream);
+
 /* Diagnostic: measured FP64 throughput of the current device in TFLOP/s, from chains of independent
  * DFMA instructions and of DMMA (mma.sync.m8n8k4.f64) instructions; used as the roofline denominator
  * of the FP64-bound block kernels.  Synchronous; takes a few milliseconds. */

@@ -11,6 +11,8 @@ from .binding import (  # noqa: F401
     NegfError,
     EXPORTED_SYMBOLS,
     load_library,
+    broyden_residual_noalloc,
+    NEGF_NOALLOC_MAX_LEN,
     negf_fp64_peak,
     negf_version,
 )

@@ -27,7 +27,7 @@ EXPORTED_SYMBOLS = [
     "negf_create", "negf_destroy", "negf_set_potential", "negf_charge", "negf_transmission",
     "negf_self_energy", "negf_current", "negf_set_probe", "negf_integrand_peak", "negf_solve_host", "negf_sync",
     "negf_kernel_stats", "negf_get_plan",
-    "broyden_create", "broyden_step", "broyden_reset", "broyden_destroy",
+    "broyden_create", "broyden_step", "broyden_reset", "broyden_destroy", "broyden_residual_noalloc",
     "negf_fp64_peak", "negf_last_error", "negf_version",
 ]
 
@@ -100,6 +100,7 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
         "broyden_step": (C.c_int, [vp, vp, vp, C.POINTER(dbl)]),
         "broyden_reset": (C.c_int, [vp]),
         "broyden_destroy": (C.c_int, [vp]),
+        "broyden_residual_noalloc": (C.c_int, [vp, vp, i64, vp, vp]),
         "negf_fp64_peak": (C.c_int, [C.POINTER(dbl), C.POINTER(dbl)]),
         "negf_last_error": (C.c_char_p, []),
         "negf_version": (C.c_char_p, []),
@@ -316,6 +317,19 @@ class Broyden:
             self.broyden_destroy()
         except Exception:
             pass
+
+
+NEGF_NOALLOC_MAX_LEN = 1 << 26      # include/negf.h
+
+
+def broyden_residual_noalloc(x_in_dev, x_out_dev, eps_max_dev, length: Optional[int] = None, stream=None):
+    """``broyden_residual_noalloc`` (include/negf.h): eps_max of Alg.3 steps 4-7 into the one-element
+    device tensor ``eps_max_dev``; launches on ``stream``, allocates nothing, does not synchronise."""
+    n = int(x_in_dev.numel() if length is None else length)
+    need = n if 1 <= n <= NEGF_NOALLOC_MAX_LEN else 0       # out-of-range lengths are refused by the library
+    _check(load_library().broyden_residual_noalloc(
+        _dev_ptr(x_in_dev, need, "x_in_dev"), _dev_ptr(x_out_dev, need, "x_out_dev"), n,
+        _dev_ptr(eps_max_dev, 1, "eps_max_dev"), _stream_ptr(stream)), "broyden_residual_noalloc")
 
 
 def negf_fp64_peak():
