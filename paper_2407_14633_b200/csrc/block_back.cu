@@ -2,7 +2,7 @@
 // the column recursion of Algorithm 1 steps 2-3 and 6-8 from the last lead k,
 //     C_{N-1} = g_{N-1} F_k,   C_s = ytilde_s C_{s+1},   Tr A_k,(i,i) = ||C_s||_F^2,
 //     T = ||F_first^dagger C_0||_F^2   (eq.(5)),
-// with ytilde_s read from the history that block_sweep_kernel<17> wrote.
+// with ytilde_s read from the history that block_fwd17_kernel wrote.
 //
 // This half of the sweep is a plain 17 x 17 complex product per ring with no pivoting, i.e. a dense
 // contraction once the 17th row and column are split off: the 16 x 16 x 16 core is 2 x 2 output
@@ -12,10 +12,11 @@
 // so the gain is not peak: it is one issue slot per 256 FMAs instead of 8, and one 8-byte operand per
 // lane per 128 FMAs instead of one 16-byte operand per 8, which is what bounded the SIMT version.
 //
-// One warp per half-sweep task, 7 warps per CTA (the 7 tasks of one block_sweep CTA, whose partial-
+// One warp per half-sweep task, 8 warps per CTA (the 8 tasks of one block_fwd17 CTA, whose partial-
 // charge row they share); no barrier inside a ring.  The history of a task and ring is the row-major
 // matrix ytilde_s with row stride 18 (rows start on 32-byte sectors); A fragment (mt, ks) of lane l is
 // element [8 mt + l/4][4 ks + l%4]: four lanes read one aligned 64-byte piece, 16 full sectors per load.
+#include "block_ops17.cuh"
 #include "block_ops2.cuh"
 #include "block_path.h"
 #include "negf_internal.h"
@@ -63,7 +64,7 @@ __device__ __forceinline__ CtaId17 decode_real_cta(const SweepLaunch& p, long lo
 
 __global__ void __launch_bounds__(kBackThreads17, 2) block_back17_kernel(const SweepLaunch p, long long first_gid) {
   using G = Geo2<NB17>;
-  constexpr int TPC = G::TPC;                       // 7 tasks = 7 warps
+  constexpr int TPC = kTpc17;                       // 8 tasks = 8 warps
   constexpr long long STEP = G::STEP_ELEMS;
   constexpr int MAT = NB17 * NB17;
   __shared__ __align__(16) c64 Bs_all[TPC][NB17 * LDB];
@@ -205,7 +206,7 @@ __global__ void __launch_bounds__(kBackThreads17, 2) block_back17_kernel(const S
     }
     if (lane == 0) Bs[16 * LDB + 16] = cornv;
 
-    // ---- first stage of eq.(4): every 32 rings the CTA sums its 7 tasks (fixed order)
+    // ---- first stage of eq.(4): every 32 rings the CTA sums its 8 tasks (fixed order)
     if ((cnt & 31) == 31 || s == 0) {
       red[t][lane] = keep;
       keep = 0.0;

@@ -1,0 +1,299 @@
+// Forward half of the block RGF sweep for n = 17, real-axis energies (step a2 of SURVEY.md 8(a);
+// Algorithm 2 of PAPER.md:121-141 for the connected Green's functions ytilde_s):
+//     d_s = z - U_s - K_s ytilde_{s-1} (- Sigma at the two ends),  g_s = d_s^-1,
+//     ytilde_s = g_s K_{s+1}^dagger   (stored as written: the way back, block_back.cu, reads it),
+// one half-sweep task (channel, energy, direction) per EIGHT lanes: four tasks per warp, eight per CTA,
+// no CTA barrier and no shared-memory pivot traffic inside a ring (block_ops17.cuh).  A warp owns its four
+// tasks for the whole sweep; the two warps of a CTA only share the coupling tables.
+//
+// CTA numbering, history layout (row-major records of kHistRec17 elements per task and ring, row stride
+// 18) and the table of lead self-energies are those of block_sweep.cu / block_back.cu; a real-axis CTA of
+// n = 17 holds kTpc17 = 8 consecutive energies.
+#include "block_ops17.cuh"
+#include "block_ops2.cuh"
+#include "block_path.h"
+#include "negf_internal.h"
+
+namespace negf {
+namespace blk {
+
+namespace {
+
+constexpr int NB = 17;
+constexpr int MAT = NB * NB;
+constexpr int kFwdThreads17 = 64;
+
+__device__ __forceinline__ void st32(c64* dst, c64 a, c64 b) {          // one full 32-byte sector
+  asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(dst), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y)
+               : "memory");
+}
+// a row of ytilde_s: 17 elements + the padding element, nine full sectors
+__device__ __forceinline__ void store_row17(c64* dst, const c64 (&row)[NB]) {
+#pragma unroll
+  for (int j = 0; j < 8; ++j) st32(dst + 2 * j, row[2 * j], row[2 * j + 1]);
+  st32(dst + 16, row[16], make_double2(0.0, 0.0));
+}
+
+// rows l8, l8 + 8 and the lane's share of row 16 of  -K X   (X: the task's matrix in shared memory)
+__device__ __forceinline__ void sparse_left17(c64 (&R)[2][NB], c64 (&S)[3], const CsrS K, unsigned X, int l8) {
+#pragma unroll
+  for (int q = 0; q < 2; ++q) {
+#pragma unroll
+    for (int b = 0; b < NB; ++b) R[q][b] = make_double2(0.0, 0.0);
+    const int rid = l8 + 8 * q;
+    const int e0 = lds_i32(K.rowptr + 4 * rid), e1 = lds_i32(K.rowptr + 4 * rid + 4);
+#pragma unroll 1
+    for (int e = e0; e < e1; ++e) {
+      const c64 v = lds_c64(K.val + 16 * e);
+      const unsigned xr = X + (unsigned)lds_i32(K.col + 4 * e) * (NB * 16);
+#pragma unroll
+      for (int b = 0; b < NB; ++b) cfms(R[q][b], v, lds_c64(xr + 16 * b));
+    }
+  }
+  S[0] = S[1] = S[2] = make_double2(0.0, 0.0);
+  const int e0 = lds_i32(K.rowptr + 4 * 16), e1 = lds_i32(K.rowptr + 4 * 17);
+#pragma unroll 1
+  for (int e = e0; e < e1; ++e) {
+    const c64 v = lds_c64(K.val + 16 * e);
+    const unsigned xr = X + (unsigned)lds_i32(K.col + 4 * e) * (NB * 16);
+    cfms(S[0], v, lds_c64(xr + 16 * l8));
+    cfms(S[1], v, lds_c64(xr + 16 * (l8 + 8)));
+    cfms(S[2], v, lds_c64(xr + 16 * 16));
+  }
+}
+
+// the same rows of  X K^dagger:  (X K^dagger)[r][b] = sum_{d in nz(K_b)} X[r][d] conj(K[b][d])
+__device__ __forceinline__ void sparse_right_dagger17(c64 (&R)[2][NB], c64 (&S)[3], const CsrS K, unsigned X,
+                                                      int l8) {
+  const unsigned x0 = X + l8 * (NB * 16), x1 = X + (l8 + 8) * (NB * 16), x16 = X + 16 * (NB * 16);
+#pragma unroll
+  for (int b = 0; b < NB; ++b) {
+    c64 acc0 = make_double2(0.0, 0.0), acc1 = make_double2(0.0, 0.0);
+    const int e0 = lds_i32(K.rowptr + 4 * b), e1 = lds_i32(K.rowptr + 4 * b + 4);
+#pragma unroll 1
+    for (int e = e0; e < e1; ++e) {
+      const c64 kv = cconj(lds_c64(K.val + 16 * e));
+      const unsigned cidx = 16u * (unsigned)lds_i32(K.col + 4 * e);
+      cfma(acc0, lds_c64(x0 + cidx), kv);
+      cfma(acc1, lds_c64(x1 + cidx), kv);
+    }
+    R[0][b] = acc0;
+    R[1][b] = acc1;
+  }
+#pragma unroll
+  for (int x = 0; x < 3; ++x) {
+    const int b = x == 0 ? l8 : x == 1 ? l8 + 8 : 16;
+    c64 acc = make_double2(0.0, 0.0);
+    const int e0 = lds_i32(K.rowptr + 4 * b), e1 = lds_i32(K.rowptr + 4 * b + 4);
+#pragma unroll 1
+    for (int e = e0; e < e1; ++e)
+      cfma(acc, lds_c64(x16 + 16u * (unsigned)lds_i32(K.col + 4 * e)), cconj(lds_c64(K.val + 16 * e)));
+    S[x] = acc;
+  }
+}
+
+// the task's matrix (registers, layout of block_ops17.cuh) to its shared-memory matrix, row-major
+__device__ __forceinline__ void to_shared17(c64* mat_t, const c64 (&R)[2][NB], const c64 (&S)[3], int l8) {
+#pragma unroll
+  for (int q = 0; q < 2; ++q)
+#pragma unroll
+    for (int b = 0; b < NB; ++b) mat_t[(l8 + 8 * q) * NB + b] = R[q][b];
+  mat_t[16 * NB + l8] = S[0];
+  mat_t[16 * NB + l8 + 8] = S[1];
+  if (l8 == 0) mat_t[16 * NB + 16] = S[2];
+}
+
+size_t fwd17_smem(int nnz_cap) {
+  return sizeof(c64) * kTpc17 * MAT + 2 * csr_shared_bytes(NB, nnz_cap) + 2 * NB * sizeof(c64) + 32;
+}
+
+}  // namespace
+
+__global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const SweepLaunch p, long long first_gid) {
+  constexpr long long STEP = Geo2<NB>::STEP_ELEMS;
+  extern __shared__ __align__(16) char smem_raw[];
+  c64* mat = reinterpret_cast<c64*>(smem_raw);                    // [kTpc17][17 x 17]
+  char* nxt = smem_raw + sizeof(c64) * kTpc17 * MAT;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int l8 = lane & 7, base = lane & 24, t = tid >> 3;
+  const int N = p.N;
+  const long long gid = first_gid + blockIdx.x;
+  // real-axis CTA numbering of block_sweep.cu: after the contour CTAs, (channel, group, direction)
+  const long long rr = gid - p.n_eq_cta;
+  const int per = 2 * p.gneq;
+  const int c = (int)(rr / per);
+  const int rem = (int)(rr - (long long)c * per);
+  const int grp = rem >> 1, dir = rem & 1;
+  int k = grp * kTpc17 + t;
+  if (k >= p.K_neq) k = p.K_neq - 1;       // a padding task repeats the last energy; nobody reads its history
+  const c64 z = p.z_neq[k];
+  const size_t K_all = (size_t)p.K_eq + p.K_neq;
+  const size_t tab_off = (((size_t)c * K_all + p.K_eq + k) * 2 + 0) * 2 * MAT;
+#define NEGF_TAB_FIRST (p.table + tab_off + (dir ? 2 * MAT : 0))
+#define NEGF_TAB_LAST (p.table + tab_off + (dir ? 0 : 2 * MAT))
+
+  // couplings of this direction, by parity of the bond: [0] even bond, [1] odd bond (as in block_sweep.cu)
+  Csr Kgen[2];
+  CsrS Kpar[2];
+  c64* kd[2];
+  bool kdiag[2];
+  {
+    const int m0 = dir ? CSR_E : CSR_EDAG, m1 = dir ? CSR_O : CSR_ODAG;
+    nxt = csr_to_shared(Kgen[0], nxt, p.csr.rowptr + m0 * (NB + 1), p.csr.col + (size_t)m0 * p.csr.nnz_cap,
+                        p.csr.val + (size_t)m0 * p.csr.nnz_cap, NB, p.csr.nnz_cap);
+    nxt = csr_to_shared(Kgen[1], nxt, p.csr.rowptr + m1 * (NB + 1), p.csr.col + (size_t)m1 * p.csr.nnz_cap,
+                        p.csr.val + (size_t)m1 * p.csr.nnz_cap, NB, p.csr.nnz_cap);
+    Kpar[0] = csr_shared(Kgen[0]);
+    Kpar[1] = csr_shared(Kgen[1]);
+    kd[0] = reinterpret_cast<c64*>(nxt);
+    kd[1] = kd[0] + NB;
+    for (int i = tid; i < NB; i += kFwdThreads17) {
+      kd[0][i] = p.csr.diag[m0 * NB + i];
+      kd[1][i] = p.csr.diag[m1 * NB + i];
+    }
+    kdiag[0] = (p.csr.diag_mask >> m0) & 1;
+    kdiag[1] = (p.csr.diag_mask >> m1) & 1;
+  }
+  __syncthreads();                          // the only CTA barrier: from here every warp runs on its own
+
+  c64* mat_t = mat + (size_t)t * MAT;
+  const unsigned mat_s = smem_addr(mat_t);
+  c64* hrec = p.hist + (size_t)(gid - p.cta_begin) * N * STEP + (size_t)t * kHistRec17;   // + s * STEP
+  const double* Uc = p.U + (size_t)c * N;
+  double u_next = Uc[dir ? N - 1 : 0];      // potential of the next ring, loaded one ring ahead
+
+  // Loop invariant at the top of step s > 0: R, S = the lane's share of ytilde_{s-1}; if the coupling
+  // entering step s is not diagonal, ytilde_{s-1} is also in the task's shared-memory matrix.
+  c64 R[2][NB], S[3];
+  for (int s = 0; s < N; ++s) {
+    const int i = dir ? N - 1 - s : s;
+    const double zu = z.x - u_next;
+    if (s < N - 1) u_next = Uc[dir ? i - 1 : i + 1];
+    if (s == 0) {
+      const c64* tab = NEGF_TAB_FIRST;
+#pragma unroll
+      for (int q = 0; q < 2; ++q)
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+          const c64 v = tab[(l8 + 8 * q) * NB + b];
+          R[q][b] = make_double2(-v.x, -v.y);
+        }
+      const c64 v0 = tab[16 * NB + l8], v1 = tab[16 * NB + l8 + 8], v2 = tab[16 * NB + 16];
+      S[0] = make_double2(-v0.x, -v0.y);
+      S[1] = make_double2(-v1.x, -v1.y);
+      S[2] = make_double2(-v2.x, -v2.y);
+    } else {
+      const int par = dir ? (i & 1) : ((i - 1) & 1);
+      // d := -K_s ytilde_{s-1}
+      if (kdiag[par]) {
+        const c64* kdp = kd[par];
+        const c64 k0 = kdp[l8], k1 = kdp[l8 + 8], k2 = kdp[16];
+        const c64 n0 = make_double2(-k0.x, -k0.y), n1 = make_double2(-k1.x, -k1.y);
+        const c64 n2 = make_double2(-k2.x, -k2.y);
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+          R[0][b] = cmul(n0, R[0][b]);
+          R[1][b] = cmul(n1, R[1][b]);
+        }
+        S[0] = cmul(n2, S[0]);
+        S[1] = cmul(n2, S[1]);
+        S[2] = cmul(n2, S[2]);
+      } else {
+        sparse_left17(R, S, Kpar[par], mat_s, l8);
+      }
+    }
+    if (s == N - 1) {
+      const c64* tab = NEGF_TAB_LAST;
+#pragma unroll
+      for (int q = 0; q < 2; ++q)
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+          const c64 v = tab[(l8 + 8 * q) * NB + b];
+          R[q][b].x -= v.x;
+          R[q][b].y -= v.y;
+        }
+      const c64 v0 = tab[16 * NB + l8], v1 = tab[16 * NB + l8 + 8], v2 = tab[16 * NB + 16];
+      S[0].x -= v0.x; S[0].y -= v0.y;
+      S[1].x -= v1.x; S[1].y -= v1.y;
+      S[2].x -= v2.x; S[2].y -= v2.y;
+    }
+#pragma unroll
+    for (int b = 0; b < 8; ++b)
+      if (b == l8) {
+        R[0][b].x += zu; R[0][b].y += z.y;
+        R[1][b + 8].x += zu; R[1][b + 8].y += z.y;
+      }
+    S[2].x += zu;
+    S[2].y += z.y;
+
+    __syncwarp();                            // the shared-memory matrix is free (scratch of the inversion)
+    invert17_w8(R, S, p.theta2, l8, base, mat_t, NB);
+
+    int parn = 0;
+    bool next_diag = false;
+    if (s < N - 1) {
+      const int inext = dir ? i - 1 : i + 1;
+      parn = dir ? (inext & 1) : ((inext - 1) & 1);
+      next_diag = kdiag[parn];
+    }
+    c64* h = hrec + (size_t)s * STEP;
+    if (s == N - 1 || next_diag) {
+      if (s < N - 1) {                       // ytilde_ab = g_ab conj(K_bb); last ring: G_(k,k) itself
+        const c64* kdn = kd[parn];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+          const c64 kb = cconj(kdn[b]);
+          R[0][b] = cmul(R[0][b], kb);
+          R[1][b] = cmul(R[1][b], kb);
+        }
+        S[0] = cmul(S[0], cconj(kdn[l8]));
+        S[1] = cmul(S[1], cconj(kdn[l8 + 8]));
+        S[2] = cmul(S[2], cconj(kdn[16]));
+      }
+      mat_t[16 * NB + l8] = S[0];            // row 16 goes out through shared memory: full sectors
+      mat_t[16 * NB + l8 + 8] = S[1];
+      if (l8 == 0) mat_t[16 * NB + 16] = S[2];
+    } else {
+      to_shared17(mat_t, R, S, l8);
+      __syncwarp();
+      sparse_right_dagger17(R, S, Kpar[parn], mat_s, l8);   // ytilde_s = g_s K_{s+1}^dagger
+      __syncwarp();                          // g has been read by everyone
+      to_shared17(mat_t, R, S, l8);
+    }
+    __syncwarp();
+    store_row17(h + l8 * kHistLd17, R[0]);
+    store_row17(h + (l8 + 8) * kHistLd17, R[1]);
+    {
+      const c64* r16 = mat_t + 16 * NB;
+      st32(h + 16 * kHistLd17 + 2 * l8, r16[2 * l8], r16[2 * l8 + 1]);
+      if (l8 == 0) st32(h + 16 * kHistLd17 + 16, r16[16], make_double2(0.0, 0.0));
+    }
+  }
+#undef NEGF_TAB_FIRST
+#undef NEGF_TAB_LAST
+}
+
+cudaError_t launch_block_fwd17(const SweepLaunch& p, cudaStream_t s) {
+  // real-axis CTAs of this launch: global ids [max(cta_begin, n_eq_cta), cta_begin + n_cta)
+  const long long first = p.cta_begin > p.n_eq_cta ? p.cta_begin : p.n_eq_cta;
+  const long long n = p.cta_begin + p.n_cta - first;
+  if (n <= 0) return cudaSuccess;
+  const size_t smem = fwd17_smem(p.csr.nnz_cap);
+  cudaError_t e = cudaFuncSetAttribute(block_fwd17_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  block_fwd17_kernel<<<(unsigned)n, kFwdThreads17, smem, s>>>(p, first);
+  return cudaGetLastError();
+}
+
+int block_fwd17_ctas_per_sm(int nnz_cap) {
+  int nb = 0;
+  const size_t smem = fwd17_smem(nnz_cap);
+  if (cudaFuncSetAttribute(block_fwd17_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, block_fwd17_kernel, kFwdThreads17, smem) != cudaSuccess)
+    return 0;
+  return nb;
+}
+
+}  // namespace blk
+}  // namespace negf

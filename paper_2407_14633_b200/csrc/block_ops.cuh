@@ -261,6 +261,26 @@ __device__ __forceinline__ char* csr_to_shared(Csr& dst, char* base, const int* 
   char* end = reinterpret_cast<char*>(col + nnz_cap);
   return reinterpret_cast<char*>((reinterpret_cast<uintptr_t>(end) + 15) & ~uintptr_t(15));
 }
+// Explicit shared-memory loads (32-bit shared addresses): the CSR tables are reached through
+// pointers selected at run time, for which the compiler otherwise falls back to generic loads.
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ int lds_i32(unsigned addr) {
+  int v;
+  asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ c64 lds_c64(unsigned addr) {
+  c64 v;
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+  return v;
+}
+struct CsrS {            // CSR matrix in shared memory, by shared address
+  unsigned rowptr, col, val;
+};
+__device__ __forceinline__ CsrS csr_shared(const Csr& K) {
+  return CsrS{smem_addr(K.rowptr), smem_addr(K.col), smem_addr(K.val)};
+}
+
 __host__ __device__ constexpr size_t csr_shared_bytes(int nb, int nnz_cap) {
   return ((sizeof(double2) * (size_t)nnz_cap + sizeof(int) * (size_t)(nb + 1 + nnz_cap)) + 15) / 16 * 16;
 }

@@ -26,9 +26,10 @@ struct Geo2 {
   static constexpr int MAT = NB * NB;
   static constexpr int PROW = NB + 1;                                // pivot row + reciprocal pivot
   // one ring step of recursion history of one CTA: [slot q][column b][thread] complex; for n = 17 the
-  // real-axis CTAs store, in the same space, TPC row-major matrices of kHistRec17 elements (block_back.cu)
-  static constexpr long long STEP_ELEMS = 2LL * NB * THREADS;
-  static_assert(NB != 17 || TPC * 306 <= 2 * NB * THREADS, "row-major records must fit the step");
+  // real-axis CTAs (block_fwd17.cu) store, in the same space, row-major matrices of kHistRec17 elements
+  // (n = 17: 8 records of 306, the 8 tasks of a block_fwd17 CTA; the contour CTAs use the first 2176)
+  static constexpr long long STEP_ELEMS = NB == 17 ? 8LL * 306 : 2LL * NB * THREADS;
+  static_assert(STEP_ELEMS >= 2LL * NB * THREADS, "the contour layout must fit the step");
 };
 
 template <int NB>

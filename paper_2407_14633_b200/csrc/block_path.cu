@@ -208,7 +208,8 @@ negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, c
   bp->tpc = blk::block_tasks_per_cta(n);
   bp->threads = blk::block_threads(n);
   bp->geq = (bp->K_eq + bp->tpc - 1) / bp->tpc;
-  bp->gneq = (bp->K_neq + bp->tpc - 1) / bp->tpc;
+  const int tpc_real = blk::block_tasks_per_cta_real(n);
+  bp->gneq = (bp->K_neq + tpc_real - 1) / tpc_real;
   bp->n_eq_cta = (long long)bp->C * bp->geq * 2;
   bp->total_cta = (long long)bp->C * 2 * (bp->geq + bp->gneq);
   const size_t K_all = (size_t)bp->K_eq + bp->K_neq;
@@ -259,10 +260,13 @@ negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, c
   {
     const char* force = getenv("NEGF_FORCE_OVERLAP");   // test hook: "1" forces the plan on small devices, "0" forbids it
     const bool possible = bp->C == 1 && bp->n_launches == 1 && bp->n_eq_cta > 0 && bp->total_cta > bp->n_eq_cta;
-    const bool pays = bp->total_cta > bp->wave && bp->total_cta - bp->n_eq_cta <= bp->wave;
+    // n = 17: the contour and the real-axis CTAs are different kernels (block_sweep.cu, block_fwd17.cu), so
+    // the contour sweep always gains from running beside the self-energies of the real-axis energies
+    const bool pays = bp->n == 17 || (bp->total_cta > bp->wave && bp->total_cta - bp->n_eq_cta <= bp->wave);
     bp->overlap = possible && (force ? force[0] == '1' : pays);
   }
-  if (bp->overlap) {
+  if (bp->overlap || bp->n == 17) {
+    // (n = 17 without the overlap plan: block_path_run puts the contour CTAs of a launch on the side stream)
     // highest priority: when the contour CTAs and the second Sancho-Rubio launch become ready together, the
     // few contour CTAs must be placed first (a Sancho-Rubio CTA takes a whole SM's registers)
     int prio_lo = 0, prio_hi = 0;
@@ -389,11 +393,33 @@ negf_status block_path_run(BlockPath* bp, const double* U_dev, double* n_res, do
     for (long long begin = 0; begin < bp->total_cta; begin += bp->slots) {
       p.cta_begin = begin;
       p.n_cta = (int)std::min<long long>(bp->slots, bp->total_cta - begin);
+      const long long eq_end = std::min<long long>(begin + p.n_cta, bp->n_eq_cta);
+      if (bp->n == 17 && eq_end > begin && begin + p.n_cta > bp->n_eq_cta) {
+        // n = 17, a launch with both kinds of CTA: two kernels, which must not run one after the other (the
+        // few contour CTAs would hold the device for a whole sweep).  Contour CTAs + combine go to the side
+        // stream, the real-axis CTAs stay here in the slots after them; joined before the slots are reused.
+        NEGF_CUDA_TRY(cudaEventRecord(bp->ev_fork, s));
+        NEGF_CUDA_TRY(cudaStreamWaitEvent(bp->side, bp->ev_fork, 0));
+        blk::SweepLaunch q = p;
+        q.n_cta = (int)(eq_end - begin);
+        NEGF_CUDA_TRY(blk::launch_block_sweep(bp->n, q, bp->side));
+        NEGF_CUDA_TRY(blk::launch_block_combine(bp->n, q, begin, (int)((eq_end - begin) / 2), bp->side));
+        NEGF_CUDA_TRY(cudaEventRecord(bp->ev_join, bp->side));
+        blk::SweepLaunch r = p;
+        r.cta_begin = eq_end;
+        r.n_cta = (int)(begin + p.n_cta - eq_end);
+        r.hist = p.hist + (size_t)(eq_end - begin) * bp->N * blk::block_step_elems(bp->n);
+        hook.begin(hook.ctx, 1);
+        cudaError_t e2 = blk::launch_block_sweep(bp->n, r, s);
+        hook.end(hook.ctx);
+        NEGF_CUDA_TRY(e2);
+        NEGF_CUDA_TRY(cudaStreamWaitEvent(s, bp->ev_join, 0));
+        continue;
+      }
       hook.begin(hook.ctx, 1);
       cudaError_t e = blk::launch_block_sweep(bp->n, p, s);
       hook.end(hook.ctx);
       NEGF_CUDA_TRY(e);
-      const long long eq_end = std::min<long long>(begin + p.n_cta, bp->n_eq_cta);
       if (eq_end > begin) {
         hook.begin(hook.ctx, 3);
         e = blk::launch_block_combine(bp->n, p, begin, (int)((eq_end - begin) / 2), s);
@@ -441,11 +467,12 @@ void block_path_plan(BlockPath* bp, negf_plan_info* out) {
   out->n_batches = bp->n_launches;
   out->max_sr_iterations = bp->last_max_iters;
   out->sr_passes_total = bp->last_sr_passes;
-  // negate + Sancho-Rubio + sweep kernels (n = 17: forward + way-back kernel when the launch holds real-axis
-  // CTAs) + one combine per launch that holds contour CTAs + 2-level reduce
+  // negate + Sancho-Rubio + sweep kernels (n = 17: one for the contour CTAs of a launch, forward + way-back
+  // kernel for its real-axis CTAs) + one combine per launch that holds contour CTAs + 2-level reduce
   int sweeps = 0, combines = 0;
   for (long long b = 0; b < bp->total_cta; b += bp->slots) {
-    sweeps += (bp->n == 17 && b + bp->slots > bp->n_eq_cta) ? 2 : 1;
+    if (bp->n == 17) sweeps += (b < bp->n_eq_cta ? 1 : 0) + (b + bp->slots > bp->n_eq_cta ? 2 : 0);
+    else ++sweeps;
     if (b < bp->n_eq_cta) ++combines;
   }
   // overlap plan: two Sancho-Rubio launches and a contour sweep launch of its own

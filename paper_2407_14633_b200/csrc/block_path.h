@@ -93,14 +93,17 @@ cudaError_t launch_block_sweep(int nb, const SweepLaunch& p, cudaStream_t s);
 // (block_back.cu).  Other block sizes do the way back inside block_sweep_kernel.
 constexpr int kHistLd17 = 18;         // row stride of a history matrix: 288 B rows start on 32-byte sectors
 constexpr int kHistRec17 = 17 * kHistLd17;   // history elements per task and ring
-constexpr int kBackThreads17 = 224;   // 7 warps = the 7 tasks of one block_sweep CTA
+constexpr int kBackThreads17 = 256;   // 8 warps = the 8 tasks of one block_fwd17 CTA
 cudaError_t launch_block_back17(const SweepLaunch& p, cudaStream_t s);
+cudaError_t launch_block_fwd17(const SweepLaunch& p, cudaStream_t s);    // block_fwd17.cu
+int block_fwd17_ctas_per_sm(int nnz_cap);
 // Contour combine over the pairs of contour CTAs [cta_begin, cta_begin + 2 n_pairs) of a finished
 // sweep launch whose first CTA was launch_cta_begin.
 cudaError_t launch_block_combine(int nb, const SweepLaunch& p, long long pair_cta_begin, int n_pairs,
                                  cudaStream_t s);
 // Geometry queries (host).
 int block_tasks_per_cta(int nb);
+int block_tasks_per_cta_real(int nb);   // real-axis CTAs (n = 17: block_fwd17.cu holds 8)
 int block_threads(int nb);
 long long block_step_elems(int nb);   // history elements per ring step per CTA
 size_t block_sweep_smem(int nb, int nnz_cap);

@@ -12,6 +12,7 @@
 //     Tr A_k,(i,i) = ||C_s||_F^2,   T = ||F_first^dagger C_0||_F^2   (eq.(5))
 // Contour points need Tr G_(i,i) = Tr [alpha_i - x_i - y_i]^-1 (Alg.1 step 1): their two half-sweeps
 // store x_i / y_i = K_s ytilde_{s-1} and a second kernel (parallel over rings) inverts and traces.
+#include "block_ops17.cuh"
 #include "block_ops2.cuh"
 #include "block_path.h"
 #include "negf_internal.h"
@@ -36,26 +37,6 @@ __device__ __forceinline__ CtaId decode_cta(const SweepLaunch& p, long long gid)
   id.grp = rem >> 1;
   id.dir = rem & 1;
   return id;
-}
-
-// Explicit shared-memory loads (32-bit shared addresses): the CSR tables are reached through
-// pointers selected at run time, for which the compiler otherwise falls back to generic loads.
-__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ int lds_i32(unsigned addr) {
-  int v;
-  asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(addr));
-  return v;
-}
-__device__ __forceinline__ c64 lds_c64(unsigned addr) {
-  c64 v;
-  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
-  return v;
-}
-struct CsrS {            // CSR matrix in shared memory, by shared address
-  unsigned rowptr, col, val;
-};
-__device__ __forceinline__ CsrS csr_shared(const Csr& K) {
-  return CsrS{smem_addr(K.rowptr), smem_addr(K.col), smem_addr(K.val)};
 }
 
 // y[q][b] = - sum_{c in nz(K_rid)} K[rid][c] * X[c][b] for the thread's two rows (X in shared memory)
@@ -571,7 +552,15 @@ static int ctas_per_sm_t(int nnz_cap) {
 
 cudaError_t launch_block_sweep(int nb, const SweepLaunch& p, cudaStream_t s) {
   if (nb == 17) {
-    cudaError_t e = launch_sweep_t<17>(p, s);
+    // contour CTAs of the range: this file's kernel; real-axis CTAs: block_fwd17.cu, then block_back.cu
+    const long long eq_end = p.cta_begin + p.n_cta < p.n_eq_cta ? p.cta_begin + p.n_cta : p.n_eq_cta;
+    if (eq_end > p.cta_begin) {
+      SweepLaunch q = p;
+      q.n_cta = (int)(eq_end - p.cta_begin);
+      cudaError_t e = launch_sweep_t<17>(q, s);
+      if (e != cudaSuccess) return e;
+    }
+    cudaError_t e = launch_block_fwd17(p, s);
     return e != cudaSuccess ? e : launch_block_back17(p, s);
   }
   switch (nb) {
@@ -598,6 +587,7 @@ int block_tasks_per_cta(int nb) {
     default: return 0;
   }
 }
+int block_tasks_per_cta_real(int nb) { return nb == 17 ? kTpc17 : block_tasks_per_cta(nb); }
 int block_threads(int nb) {
   switch (nb) {
 #define NEGF_CASE(NB_) case NB_: return Geo2<NB_>::THREADS;
@@ -615,6 +605,10 @@ size_t block_sweep_smem(int nb, int nnz_cap) {
   }
 }
 int block_sweep_ctas_per_sm(int nb, int nnz_cap) {
+  if (nb == 17) {                      // both forward kernels must fit; the real-axis one carries the load
+    const int a = ctas_per_sm_t<17>(nnz_cap), b = block_fwd17_ctas_per_sm(nnz_cap);
+    return a < 1 ? a : b;
+  }
   switch (nb) {
 #define NEGF_CASE(NB_) case NB_: return ctas_per_sm_t<NB_>(nnz_cap);
     NEGF_BLOCK_SIZES(NEGF_CASE)

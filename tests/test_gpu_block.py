@@ -135,9 +135,11 @@ def test_real_space_equals_sum_of_modes_on_gpu():
     assert_parity(T_b, T_s, "block vs modes T(E)", rtol=2e-10)   # both sides SR/closed-form limited
 
 
-def test_workspace_tiling_gives_identical_results():
+def test_workspace_tiling_gives_identical_results(monkeypatch):
     """A small workspace cap forces several sweep launches (contour pairs and real-axis CTAs in
-    different launches); results must be bit-identical."""
+    different launches); results must be bit-identical.  (The overlap plan is switched off on both sides:
+    it groups the Sancho-Rubio tasks differently, which moves results by ~1e-12 -- the next test.)"""
+    monkeypatch.setenv("NEGF_FORCE_OVERLAP", "0")
     wl = wlmod.make_config(3, N=16, K_neq=50, K_eq=20)
     n1, T1, plan1 = _gpu_run(wl, want_plan=True)
     slot = 16 * 17 * 256 * 16
