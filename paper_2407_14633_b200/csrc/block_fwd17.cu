@@ -62,24 +62,14 @@ __device__ __forceinline__ void sparse_left17(c64 (&R)[2][NB], c64 (&S)[3], cons
   }
 }
 
-// the same rows of  X K^dagger:  (X K^dagger)[r][b] = sum_{d in nz(K_b)} X[r][d] conj(K[b][d])
+// ytilde = X K^dagger in place in the task's shared-memory matrix X, and the lane's share of it in R, S:
+//     (X K^dagger)[r][b] = sum_{d in nz(K_b)} X[r][d] conj(K[b][d]).
+// Rolled over the output column b on purpose (code size, block_ops17.cuh): an output row depends on the same
+// input row only, so a lane forms a row in its private temporary row `tmp` and then replaces the input row;
+// row 16 is spread over the lanes and held in registers until every lane has read it.
 __device__ __forceinline__ void sparse_right_dagger17(c64 (&R)[2][NB], c64 (&S)[3], const CsrS K, unsigned X,
-                                                      int l8) {
-  const unsigned x0 = X + l8 * (NB * 16), x1 = X + (l8 + 8) * (NB * 16), x16 = X + 16 * (NB * 16);
-#pragma unroll
-  for (int b = 0; b < NB; ++b) {
-    c64 acc0 = make_double2(0.0, 0.0), acc1 = make_double2(0.0, 0.0);
-    const int e0 = lds_i32(K.rowptr + 4 * b), e1 = lds_i32(K.rowptr + 4 * b + 4);
-#pragma unroll 1
-    for (int e = e0; e < e1; ++e) {
-      const c64 kv = cconj(lds_c64(K.val + 16 * e));
-      const unsigned cidx = 16u * (unsigned)lds_i32(K.col + 4 * e);
-      cfma(acc0, lds_c64(x0 + cidx), kv);
-      cfma(acc1, lds_c64(x1 + cidx), kv);
-    }
-    R[0][b] = acc0;
-    R[1][b] = acc1;
-  }
+                                                      c64* mat_t, unsigned tmp, int l8) {
+  const unsigned x16 = X + 16 * (NB * 16);
 #pragma unroll
   for (int x = 0; x < 3; ++x) {
     const int b = x == 0 ? l8 : x == 1 ? l8 + 8 : 16;
@@ -90,6 +80,28 @@ __device__ __forceinline__ void sparse_right_dagger17(c64 (&R)[2][NB], c64 (&S)[
       cfma(acc, lds_c64(x16 + 16u * (unsigned)lds_i32(K.col + 4 * e)), cconj(lds_c64(K.val + 16 * e)));
     S[x] = acc;
   }
+#pragma unroll
+  for (int q = 0; q < 2; ++q) {
+    const unsigned xr = X + (l8 + 8 * q) * (NB * 16);
+#pragma unroll 1
+    for (int b = 0; b < NB; ++b) {
+      c64 acc = make_double2(0.0, 0.0);
+      const int e0 = lds_i32(K.rowptr + 4 * b), e1 = lds_i32(K.rowptr + 4 * b + 4);
+#pragma unroll 1
+      for (int e = e0; e < e1; ++e)
+        cfma(acc, lds_c64(xr + 16u * (unsigned)lds_i32(K.col + 4 * e)), cconj(lds_c64(K.val + 16 * e)));
+      asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(tmp + 16u * b), "d"(acc.x), "d"(acc.y) : "memory");
+    }
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+      R[q][b] = lds_c64(tmp + 16u * b);
+      mat_t[(l8 + 8 * q) * NB + b] = R[q][b];
+    }
+  }
+  __syncwarp();                              // every lane has read row 16 of X
+  mat_t[16 * NB + l8] = S[0];
+  mat_t[16 * NB + l8 + 8] = S[1];
+  if (l8 == 0) mat_t[16 * NB + 16] = S[2];
 }
 
 // the task's matrix (registers, layout of block_ops17.cuh) to its shared-memory matrix, row-major
@@ -104,7 +116,9 @@ __device__ __forceinline__ void to_shared17(c64* mat_t, const c64 (&R)[2][NB], c
 }
 
 size_t fwd17_smem(int nnz_cap) {
-  return sizeof(c64) * kTpc17 * MAT + 2 * csr_shared_bytes(NB, nnz_cap) + 2 * NB * sizeof(c64) + 32;
+  // exchange matrices, one temporary row per thread, rare-path records, coupling tables and their diagonals
+  return sizeof(c64) * kTpc17 * MAT + sizeof(c64) * kFwdThreads17 * NB + sizeof(Rare17) * kTpc17 +
+         2 * csr_shared_bytes(NB, nnz_cap) + 2 * NB * sizeof(c64) + 32;
 }
 
 }  // namespace
@@ -113,7 +127,9 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
   constexpr long long STEP = Geo2<NB>::STEP_ELEMS;
   extern __shared__ __align__(16) char smem_raw[];
   c64* mat = reinterpret_cast<c64*>(smem_raw);                    // [kTpc17][17 x 17]
-  char* nxt = smem_raw + sizeof(c64) * kTpc17 * MAT;
+  c64* tmp_all = mat + kTpc17 * MAT;                              // [threads][17]
+  Rare17* rare_all = reinterpret_cast<Rare17*>(tmp_all + kFwdThreads17 * NB);
+  char* nxt = reinterpret_cast<char*>(rare_all + kTpc17);
   const int tid = threadIdx.x, lane = tid & 31;
   const int l8 = lane & 7, base = lane & 24, t = tid >> 3;
   const int N = p.N;
@@ -154,10 +170,13 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
     kdiag[0] = (p.csr.diag_mask >> m0) & 1;
     kdiag[1] = (p.csr.diag_mask >> m1) & 1;
   }
+  Rare17* rare = rare_all + t;
+  if (l8 == 0) rare->swapcol = 16;
   __syncthreads();                          // the only CTA barrier: from here every warp runs on its own
 
   c64* mat_t = mat + (size_t)t * MAT;
   const unsigned mat_s = smem_addr(mat_t);
+  const unsigned tmp_s = smem_addr(tmp_all + (size_t)tid * NB);
   c64* hrec = p.hist + (size_t)(gid - p.cta_begin) * N * STEP + (size_t)t * kHistRec17;   // + s * STEP
   const double* Uc = p.U + (size_t)c * N;
   double u_next = Uc[dir ? N - 1 : 0];      // potential of the next ring, loaded one ring ahead
@@ -227,7 +246,16 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
     S[2].y += z.y;
 
     __syncwarp();                            // the shared-memory matrix is free (scratch of the inversion)
-    invert17_w8(R, S, p.theta2, l8, base, mat_t, NB);
+    const c64 dinv16 = invert17_core(R, S, p.theta2, l8, base, mat_t, rare);
+    to_shared17(mat_t, R, S, l8);            // G, -G b d^-1 and (row 16) c
+    __syncwarp();
+    invert17_border(S, dinv16, mat_s, l8);
+    __syncwarp();
+    mat_t[16 * NB + l8] = S[0];              // the complete inverse is in shared memory
+    mat_t[16 * NB + l8 + 8] = S[1];
+    if (l8 == 0) mat_t[16 * NB + 16] = S[2];
+    __syncwarp();
+    invert17_fix_swap(R, S, mat_t, rare, l8);
 
     int parn = 0;
     bool next_diag = false;
@@ -249,16 +277,12 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
         S[0] = cmul(S[0], cconj(kdn[l8]));
         S[1] = cmul(S[1], cconj(kdn[l8 + 8]));
         S[2] = cmul(S[2], cconj(kdn[16]));
+        mat_t[16 * NB + l8] = S[0];          // row 16 goes out through shared memory: full sectors
+        mat_t[16 * NB + l8 + 8] = S[1];
+        if (l8 == 0) mat_t[16 * NB + 16] = S[2];
       }
-      mat_t[16 * NB + l8] = S[0];            // row 16 goes out through shared memory: full sectors
-      mat_t[16 * NB + l8 + 8] = S[1];
-      if (l8 == 0) mat_t[16 * NB + 16] = S[2];
     } else {
-      to_shared17(mat_t, R, S, l8);
-      __syncwarp();
-      sparse_right_dagger17(R, S, Kpar[parn], mat_s, l8);   // ytilde_s = g_s K_{s+1}^dagger
-      __syncwarp();                          // g has been read by everyone
-      to_shared17(mat_t, R, S, l8);
+      sparse_right_dagger17(R, S, Kpar[parn], mat_s, mat_t, tmp_s, l8);   // ytilde_s = g_s K_{s+1}^dagger
     }
     __syncwarp();
     store_row17(h + l8 * kHistLd17, R[0]);
