@@ -104,6 +104,22 @@ __device__ __forceinline__ void sparse_right_dagger17(c64 (&R)[2][NB], c64 (&S)[
   if (l8 == 0) mat_t[16 * NB + 16] = S[2];
 }
 
+// the lane's rows (17 columns) to the task's shared-memory matrix
+__device__ __forceinline__ void rows_to_shared17(c64* mat_t, const c64 (&R)[2][NB], int l8) {
+#pragma unroll
+  for (int q = 0; q < 2; ++q)
+#pragma unroll
+    for (int b = 0; b < NB; ++b) mat_t[(l8 + 8 * q) * NB + b] = R[q][b];
+}
+__device__ __forceinline__ void from_shared17(c64 (&R)[2][NB], c64 (&S)[3], const c64* mat_t, int l8) {
+#pragma unroll
+  for (int q = 0; q < 2; ++q)
+#pragma unroll
+    for (int b = 0; b < NB; ++b) R[q][b] = mat_t[(l8 + 8 * q) * NB + b];
+  S[0] = mat_t[16 * NB + l8];
+  S[1] = mat_t[16 * NB + l8 + 8];
+  S[2] = mat_t[16 * NB + 16];
+}
 // the task's matrix (registers, layout of block_ops17.cuh) to its shared-memory matrix, row-major
 __device__ __forceinline__ void to_shared17(c64* mat_t, const c64 (&R)[2][NB], const c64 (&S)[3], int l8) {
 #pragma unroll
@@ -171,7 +187,6 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
     kdiag[1] = (p.csr.diag_mask >> m1) & 1;
   }
   Rare17* rare = rare_all + t;
-  if (l8 == 0) rare->swapcol = 16;
   __syncthreads();                          // the only CTA barrier: from here every warp runs on its own
 
   c64* mat_t = mat + (size_t)t * MAT;
@@ -246,16 +261,21 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
     S[2].y += z.y;
 
     __syncwarp();                            // the shared-memory matrix is free (scratch of the inversion)
-    const c64 dinv16 = invert17_core(R, S, p.theta2, l8, base, mat_t, rare);
-    to_shared17(mat_t, R, S, l8);            // G, -G b d^-1 and (row 16) c
-    __syncwarp();
-    invert17_border(S, dinv16, mat_s, l8);
-    __syncwarp();
-    mat_t[16 * NB + l8] = S[0];              // the complete inverse is in shared memory
-    mat_t[16 * NB + l8 + 8] = S[1];
-    if (l8 == 0) mat_t[16 * NB + 16] = S[2];
-    __syncwarp();
-    invert17_fix_swap(R, S, mat_t, rare, l8);
+    if (__all_sync(kFullMask, invert17_first_ok(S, p.theta2))) {
+      const c64 dinv16 = invert17_core(R, S, p.theta2, l8, base, mat_t, rare);
+      rows_to_shared17(mat_t, R, l8);        // G and -G b d^-1 beside c (row 16)
+      __syncwarp();
+      invert17_border(S, dinv16, mat_s, l8);
+      __syncwarp();
+      mat_t[16 * NB + l8] = S[0];            // the complete inverse is in shared memory
+      mat_t[16 * NB + l8 + 8] = S[1];
+      if (l8 == 0) mat_t[16 * NB + 16] = S[2];
+    } else {
+      to_shared17(mat_t, R, S, l8);          // rare: partial pivoting in shared memory for the whole warp
+      __syncwarp();
+      invert17_slow(mat_t, l8);
+      from_shared17(R, S, mat_t, l8);
+    }
 
     int parn = 0;
     bool next_diag = false;

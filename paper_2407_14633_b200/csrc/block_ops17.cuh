@@ -10,9 +10,8 @@
 // and the 17th row and column are folded in by a block (Schur) step:
 //     M = [[A, b], [c, d]],   A' = A - b d^-1 c,   G = A'^-1,
 //     M^-1 = [[G, -G b d^-1], [-d^-1 c G, d^-1 + d^-1 c G b d^-1]],
-// i.e. row 16 is the FIRST pivot row.  Its pivot is d when |d|^2 >= theta^2 |row 16|^2, otherwise the
-// largest element of the row (the two columns of M are exchanged, and the two rows of M^-1 exchanged
-// back).  G is formed by the Gauss-Jordan scheme of gj_invert2 -- diagonal candidates accepted by the
+// i.e. row 16 is the FIRST pivot row, with pivot d.  When |d|^2 < theta^2 |row 16|^2 for a task (rare) its warp
+// takes a slow path instead: plain partial pivoting in shared memory (invert17_slow).  G is formed by the Gauss-Jordan scheme of gj_invert2 -- diagonal candidates accepted by the
 // row-norm test, otherwise a column search over the task's unused rows -- with -b d^-1 carried along as a
 // right-hand side, which leaves column 16 of the inverse in place.  Row 16 of the inverse, -d^-1 c G, is
 // formed from the shared-memory copy of G by a rolled loop (invert17_border): code size matters here, the
@@ -52,13 +51,11 @@ __device__ __forceinline__ int argmax8(double best, int bi) {
   return bi;
 }
 
-// Per-task bookkeeping of the rare paths, in shared memory so that the common path carries no registers
-// for them: pivot row chosen for column k (identity unless a search happened) and the column that was
-// exchanged with column 16 (16 = none).
+// Per-task bookkeeping of the column searches, in shared memory so that the common path carries no registers
+// for it: pivot row chosen for column k (identity unless a search happened).
 struct Rare17 {
   int perm[16];
-  int swapcol;
-  int pad[3];
+  int pad[4];
 };
 
 // One elimination step of the 16 x 16 Gauss-Jordan inversion: pivot row p of the lane's task, held in
@@ -74,13 +71,25 @@ __device__ __forceinline__ void gj16_eliminate(c64 (&R)[2][17], c64 pv, int p, i
   c64 f0 = cmul(R[0][0], inv), f1 = cmul(R[1][0], inv);
   if (piv0) { f0 = make_double2(0.0, 0.0); dinv[0] = inv; used[0] = true; }
   if (piv1) { f1 = make_double2(0.0, 0.0); dinv[1] = inv; used[1] = true; }
+  // the pivot row arrives by shuffle, kDepth elements ahead of their use (issued back to back with their
+  // uses, every element would expose the shuffle latency: 25 % of the kernel's stall samples)
+  constexpr int kDepth = 3;
+  c64 pj[16];
+#pragma unroll
+  for (int j = 0; j < kDepth; ++j) {
+    const c64 src = SLOT == 0 ? R[0][j + 1] : SLOT == 1 ? R[1][j + 1] : csel(pq != 0, R[1][j + 1], R[0][j + 1]);
+    pj[j] = shfl_c(src, pown);
+  }
 #pragma unroll
   for (int j = 0; j < 16; ++j) {
-    const c64 src = SLOT == 0 ? R[0][j + 1] : SLOT == 1 ? R[1][j + 1] : csel(pq != 0, R[1][j + 1], R[0][j + 1]);
-    const c64 pj = shfl_c(src, pown);
+    if (j + kDepth < 16) {
+      const int jn = j + kDepth;
+      const c64 src = SLOT == 0 ? R[0][jn + 1] : SLOT == 1 ? R[1][jn + 1] : csel(pq != 0, R[1][jn + 1], R[0][jn + 1]);
+      pj[jn] = shfl_c(src, pown);
+    }
     c64 t0 = R[0][j + 1], t1 = R[1][j + 1];
-    cfms(t0, f0, pj);
-    cfms(t1, f1, pj);
+    cfms(t0, f0, pj[j]);
+    cfms(t1, f1, pj[j]);
     if (j < 15) {
       R[0][j] = t0;
       R[1][j] = t1;
@@ -123,11 +132,18 @@ __device__ __forceinline__ void gj16_phase(c64 (&R)[2][17], const double (&thr)[
   }
 }
 
-// First part of the inversion of the task's 17 x 17 matrix (layout in the header).  On return R[q][0..15]
-// are the lane's rows of G and R[q][16] its elements of -G b d^-1 (column 16 of the inverse); S[0], S[1]
-// still hold c (after a possible column exchange, recorded in rare->swapcol); the return value is d^-1.
-// `scratch` is the task's own 17 x 17 shared-memory matrix (row-major, leading dimension 17), used only on
-// the rare paths; rare->swapcol must be 16 on entry.  Warp-synchronous: all 32 lanes call it together.
+// Whether d = M[16][16] is acceptable as the first pivot: |d|^2 >= theta^2 |row 16|^2 (per task).
+__device__ __forceinline__ bool invert17_first_ok(const c64 (&S)[3], double theta2) {
+  const double md = cabs2(S[2]);
+  const double n16 = sum8(cabs2(S[0]) + cabs2(S[1])) + md;
+  return (md >= theta2 * n16) && (md > 0.0);
+}
+
+// First part of the inversion of the task's 17 x 17 matrix (layout in the header), d being an acceptable
+// first pivot.  On return R[q][0..15] are the lane's rows of G and R[q][16] its elements of -G b d^-1 (column
+// 16 of the inverse); c has moved to row 16 of `scratch`; the return value is d^-1.  `scratch` is the task's
+// own 17 x 17 shared-memory matrix (row-major, leading dimension 17); rows 0..15 are used only when a column
+// search reordered the pivots.  Warp-synchronous: all 32 lanes call it together.
 __device__ __forceinline__ c64 invert17_core(c64 (&R)[2][17], c64 (&S)[3], double theta2, int l8, int base,
                                              c64* scratch, Rare17* rare) {
   constexpr int LD = 17;
@@ -138,38 +154,6 @@ __device__ __forceinline__ c64 invert17_core(c64 (&R)[2][17], c64 (&S)[3], doubl
 #pragma unroll
     for (int j = 0; j < 17; ++j) m = fma(R[q][j].x, R[q][j].x, fma(R[q][j].y, R[q][j].y, m));
     thr[q] = m * theta2;
-  }
-  // ---- first pivot: row 16.  d = M[16][16] if it passes the row-norm test, else the largest element of
-  // the row (columns js and 16 of M are exchanged; invert17_fix_swap exchanges rows js and 16 of the inverse)
-  {
-    const double c0 = cabs2(S[0]), c1 = cabs2(S[1]), md = cabs2(S[2]);
-    const double n16 = sum8(c0 + c1) + md;
-    const bool first = (md >= theta2 * n16) && (md > 0.0);
-    if (!__all_sync(kFullMask, first)) {
-      const int js = argmax8(c1 > c0 ? c1 : c0, c1 > c0 ? l8 + 8 : l8);
-      const c64 newd = shfl_c(csel(js >= 8, S[1], S[0]), base + (js & 7));
-      if (!first) {
-        // columns js <-> 16 of the lane's rows, through its own rows of the scratch matrix (a register
-        // array indexed by js would be demoted to local memory)
-#pragma unroll
-        for (int q = 0; q < 2; ++q) {
-          c64* mine = scratch + (l8 + 8 * q) * LD;
-#pragma unroll
-          for (int j = 0; j < 17; ++j) mine[j] = R[q][j];
-          const c64 tmp = mine[js];
-          mine[js] = mine[16];
-          mine[16] = tmp;
-#pragma unroll
-          for (int j = 0; j < 17; ++j) R[q][j] = mine[j];
-        }
-        if (l8 == (js & 7)) {
-          if (js >= 8) S[1] = S[2]; else S[0] = S[2];
-        }
-        S[2] = newd;
-        if (l8 == 0) rare->swapcol = js;
-      }
-      __syncwarp();
-    }
   }
   const c64 dinv16 = crcp(S[2]);
   {
@@ -183,6 +167,8 @@ __device__ __forceinline__ c64 invert17_core(c64 (&R)[2][17], c64 (&S)[3], doubl
     R[0][16] = make_double2(-g0.x, -g0.y);                                 // -b d^-1 rides along as column 16
     R[1][16] = make_double2(-g1.x, -g1.y);
   }
+  scratch[16 * LD + l8] = S[0];            // c waits in row 16 of the shared-memory matrix (invert17_border):
+  scratch[16 * LD + l8 + 8] = S[1];        // no registers for it during the elimination
   // ---- G = A'^-1 and G (-b d^-1)
   rare->perm[l8] = l8;
   rare->perm[l8 + 8] = l8 + 8;
@@ -240,29 +226,59 @@ __device__ __forceinline__ void invert17_border(c64 (&S)[3], c64 dinv16, unsigne
   S[2] = make_double2(dinv16.x + corner.x, dinv16.y + corner.y);
 }
 
-// Rare: a column js was exchanged with column 16 before the elimination, so rows js and 16 of the result
-// must be exchanged.  `mat` holds the complete result (17 x 17, row-major); registers are reloaded from it.
-// The caller places __syncwarp() before; warp-synchronous.
-__device__ __forceinline__ void invert17_fix_swap(c64 (&R)[2][17], c64 (&S)[3], c64* mat, Rare17* rare, int l8) {
-  const int js = rare->swapcol;
-  if (!__any_sync(kFullMask, js != 16)) return;
-  if (js != 16) {
-    for (int j = l8; j < 17; j += 8) {
-      const c64 a = mat[js * 17 + j], b = mat[16 * 17 + j];
-      mat[js * 17 + j] = b;
-      mat[16 * 17 + j] = a;
+// Slow path, taken by a whole warp when d is not acceptable as first pivot for one of its tasks (rare): plain
+// Gauss-Jordan inversion with partial pivoting of the task's matrix `m` (17 x 17, row-major, leading dimension
+// 17) in shared memory, in place, by the task's eight lanes.  Not inlined: it must not cost the fast path
+// registers.  Warp-synchronous.
+static __device__ __noinline__ void invert17_slow(c64* m, int l8) {
+  constexpr int LD = 17;
+  int piv[17];
+  for (int k = 0; k < 17; ++k) {
+    // pivot search in column k over the rows k .. 16
+    double best = -1.0;
+    int bi = k;
+    for (int i = k + l8; i < 17; i += 8) {
+      const double v = cabs2(m[i * LD + k]);
+      if (v > best) { best = v; bi = i; }
     }
+    const int p = argmax8(best, bi);
+    piv[k] = p;
+    __syncwarp();
+    if (p != k) {
+      for (int j = l8; j < 17; j += 8) {
+        const c64 a = m[k * LD + j];
+        m[k * LD + j] = m[p * LD + j];
+        m[p * LD + j] = a;
+      }
+    }
+    __syncwarp();
+    const c64 inv = crcp(m[k * LD + k]);
+    __syncwarp();
+    for (int j = l8; j < 17; j += 8) m[k * LD + j] = j == k ? inv : cmul(m[k * LD + j], inv);
+    __syncwarp();
+    for (int i = l8; i < 17; i += 8) {
+      if (i == k) continue;
+      const c64 f = m[i * LD + k];
+      for (int j = 0; j < 17; ++j) {
+        const c64 pk = m[k * LD + j];
+        c64 t = j == k ? make_double2(0.0, 0.0) : m[i * LD + j];
+        cfms(t, f, pk);
+        m[i * LD + j] = t;
+      }
+    }
+    __syncwarp();
   }
-  __syncwarp();
-#pragma unroll
-  for (int q = 0; q < 2; ++q)
-#pragma unroll
-    for (int j = 0; j < 17; ++j) R[q][j] = mat[(l8 + 8 * q) * 17 + j];
-  S[0] = mat[16 * 17 + l8];
-  S[1] = mat[16 * 17 + l8 + 8];
-  S[2] = mat[16 * 17 + 16];
-  if (l8 == 0) rare->swapcol = 16;
-  __syncwarp();
+  for (int k = 16; k >= 0; --k) {            // the row exchanges become column exchanges of the inverse
+    const int p = piv[k];
+    if (p != k) {
+      for (int i = l8; i < 17; i += 8) {
+        const c64 a = m[i * LD + k];
+        m[i * LD + k] = m[i * LD + p];
+        m[i * LD + p] = a;
+      }
+    }
+    __syncwarp();
+  }
 }
 
 }  // namespace blk
