@@ -34,16 +34,22 @@ __device__ __forceinline__ void store_row17(c64* dst, const c64 (&row)[NB]) {
   st32(dst + 16, row[16], make_double2(0.0, 0.0));
 }
 
+// A coupling matrix in shared memory as padded rows: W = row_nnz_max entries per row (value 0, column 0 where a
+// row has fewer), [17][W] values and [17][W] column indices, by shared address.  No row pointers: every row
+// loop has the same trip count, so the loads of one row are independent of each other.
+struct EllS {
+  unsigned val, col;
+};
+
 // rows l8, l8 + 8 and the lane's share of row 16 of  -K X   (X: the task's matrix in shared memory)
-__device__ __forceinline__ void sparse_left17(c64 (&R)[2][NB], c64 (&S)[3], const CsrS K, unsigned X, int l8) {
+__device__ __forceinline__ void sparse_left17(c64 (&R)[2][NB], c64 (&S)[3], const EllS K, int W, unsigned X, int l8) {
 #pragma unroll
   for (int q = 0; q < 2; ++q) {
 #pragma unroll
     for (int b = 0; b < NB; ++b) R[q][b] = make_double2(0.0, 0.0);
-    const int rid = l8 + 8 * q;
-    const int e0 = lds_i32(K.rowptr + 4 * rid), e1 = lds_i32(K.rowptr + 4 * rid + 4);
+    const int e0 = (l8 + 8 * q) * W;
 #pragma unroll 1
-    for (int e = e0; e < e1; ++e) {
+    for (int e = e0; e < e0 + W; ++e) {
       const c64 v = lds_c64(K.val + 16 * e);
       const unsigned xr = X + (unsigned)lds_i32(K.col + 4 * e) * (NB * 16);
 #pragma unroll
@@ -51,9 +57,8 @@ __device__ __forceinline__ void sparse_left17(c64 (&R)[2][NB], c64 (&S)[3], cons
     }
   }
   S[0] = S[1] = S[2] = make_double2(0.0, 0.0);
-  const int e0 = lds_i32(K.rowptr + 4 * 16), e1 = lds_i32(K.rowptr + 4 * 17);
 #pragma unroll 1
-  for (int e = e0; e < e1; ++e) {
+  for (int e = 16 * W; e < 17 * W; ++e) {
     const c64 v = lds_c64(K.val + 16 * e);
     const unsigned xr = X + (unsigned)lds_i32(K.col + 4 * e) * (NB * 16);
     cfms(S[0], v, lds_c64(xr + 16 * l8));
@@ -62,34 +67,42 @@ __device__ __forceinline__ void sparse_left17(c64 (&R)[2][NB], c64 (&S)[3], cons
   }
 }
 
+// one element of X K^dagger: sum over the W entries of row b of K of X[r][col] conj(val)   (xr: row r of X)
+template <int WT>
+__device__ __forceinline__ c64 ell_row_dot(const EllS K, int W, int b, unsigned xr) {
+  c64 acc = make_double2(0.0, 0.0);
+  if (WT > 0) {
+#pragma unroll
+    for (int w = 0; w < WT; ++w) {
+      const int e = b * WT + w;
+      cfma(acc, lds_c64(xr + 16u * (unsigned)lds_i32(K.col + 4 * e)), cconj(lds_c64(K.val + 16 * e)));
+    }
+  } else {
+#pragma unroll 1
+    for (int e = b * W; e < b * W + W; ++e)
+      cfma(acc, lds_c64(xr + 16u * (unsigned)lds_i32(K.col + 4 * e)), cconj(lds_c64(K.val + 16 * e)));
+  }
+  return acc;
+}
+
 // ytilde = X K^dagger in place in the task's shared-memory matrix X, and the lane's share of it in R, S:
 //     (X K^dagger)[r][b] = sum_{d in nz(K_b)} X[r][d] conj(K[b][d]).
 // Rolled over the output column b on purpose (code size, block_ops17.cuh): an output row depends on the same
 // input row only, so a lane forms a row in its private temporary row `tmp` and then replaces the input row;
 // row 16 is spread over the lanes and held in registers until every lane has read it.
-__device__ __forceinline__ void sparse_right_dagger17(c64 (&R)[2][NB], c64 (&S)[3], const CsrS K, unsigned X,
+template <int WT>
+__device__ __forceinline__ void sparse_right_dagger17(c64 (&R)[2][NB], c64 (&S)[3], const EllS K, int W, unsigned X,
                                                       c64* mat_t, unsigned tmp, int l8) {
   const unsigned x16 = X + 16 * (NB * 16);
-#pragma unroll
-  for (int x = 0; x < 3; ++x) {
-    const int b = x == 0 ? l8 : x == 1 ? l8 + 8 : 16;
-    c64 acc = make_double2(0.0, 0.0);
-    const int e0 = lds_i32(K.rowptr + 4 * b), e1 = lds_i32(K.rowptr + 4 * b + 4);
-#pragma unroll 1
-    for (int e = e0; e < e1; ++e)
-      cfma(acc, lds_c64(x16 + 16u * (unsigned)lds_i32(K.col + 4 * e)), cconj(lds_c64(K.val + 16 * e)));
-    S[x] = acc;
-  }
+  S[0] = ell_row_dot<WT>(K, W, l8, x16);
+  S[1] = ell_row_dot<WT>(K, W, l8 + 8, x16);
+  S[2] = ell_row_dot<WT>(K, W, 16, x16);
 #pragma unroll
   for (int q = 0; q < 2; ++q) {
     const unsigned xr = X + (l8 + 8 * q) * (NB * 16);
-#pragma unroll 1
+#pragma unroll 2
     for (int b = 0; b < NB; ++b) {
-      c64 acc = make_double2(0.0, 0.0);
-      const int e0 = lds_i32(K.rowptr + 4 * b), e1 = lds_i32(K.rowptr + 4 * b + 4);
-#pragma unroll 1
-      for (int e = e0; e < e1; ++e)
-        cfma(acc, lds_c64(xr + 16u * (unsigned)lds_i32(K.col + 4 * e)), cconj(lds_c64(K.val + 16 * e)));
+      const c64 acc = ell_row_dot<WT>(K, W, b, xr);
       asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(tmp + 16u * b), "d"(acc.x), "d"(acc.y) : "memory");
     }
 #pragma unroll
@@ -131,10 +144,12 @@ __device__ __forceinline__ void to_shared17(c64* mat_t, const c64 (&R)[2][NB], c
   if (l8 == 0) mat_t[16 * NB + 16] = S[2];
 }
 
-size_t fwd17_smem(int nnz_cap) {
-  // exchange matrices, one temporary row per thread, rare-path records, coupling tables and their diagonals
+size_t ell_bytes(int W) { return ((size_t)NB * W * (sizeof(c64) + sizeof(int)) + 15) / 16 * 16; }
+size_t fwd17_smem(int row_nnz_max) {
+  // exchange matrices, one temporary row per thread, column-search records, the two couplings as padded rows
+  // and their diagonals
   return sizeof(c64) * kTpc17 * MAT + sizeof(c64) * kFwdThreads17 * NB + sizeof(Rare17) * kTpc17 +
-         2 * csr_shared_bytes(NB, nnz_cap) + 2 * NB * sizeof(c64) + 32;
+         2 * ell_bytes(row_nnz_max) + 2 * NB * sizeof(c64) + 32;
 }
 
 }  // namespace
@@ -165,26 +180,36 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
 #define NEGF_TAB_LAST (p.table + tab_off + (dir ? 0 : 2 * MAT))
 
   // couplings of this direction, by parity of the bond: [0] even bond, [1] odd bond (as in block_sweep.cu)
-  Csr Kgen[2];
-  CsrS Kpar[2];
+  const int W = p.csr.row_nnz_max;
+  EllS Kpar[2];
   c64* kd[2];
   bool kdiag[2];
   {
-    const int m0 = dir ? CSR_E : CSR_EDAG, m1 = dir ? CSR_O : CSR_ODAG;
-    nxt = csr_to_shared(Kgen[0], nxt, p.csr.rowptr + m0 * (NB + 1), p.csr.col + (size_t)m0 * p.csr.nnz_cap,
-                        p.csr.val + (size_t)m0 * p.csr.nnz_cap, NB, p.csr.nnz_cap);
-    nxt = csr_to_shared(Kgen[1], nxt, p.csr.rowptr + m1 * (NB + 1), p.csr.col + (size_t)m1 * p.csr.nnz_cap,
-                        p.csr.val + (size_t)m1 * p.csr.nnz_cap, NB, p.csr.nnz_cap);
-    Kpar[0] = csr_shared(Kgen[0]);
-    Kpar[1] = csr_shared(Kgen[1]);
+    const int mm[2] = {dir ? CSR_E : CSR_EDAG, dir ? CSR_O : CSR_ODAG};
+#pragma unroll
+    for (int x = 0; x < 2; ++x) {
+      c64* ev = reinterpret_cast<c64*>(nxt);
+      int* ec = reinterpret_cast<int*>(ev + NB * W);
+      nxt = reinterpret_cast<char*>((reinterpret_cast<uintptr_t>(ec + NB * W) + 15) & ~uintptr_t(15));
+      const int* rp = p.csr.rowptr + mm[x] * (NB + 1);
+      const int* gc = p.csr.col + (size_t)mm[x] * p.csr.nnz_cap;
+      const c64* gv = p.csr.val + (size_t)mm[x] * p.csr.nnz_cap;
+      for (int i = tid; i < NB * W; i += kFwdThreads17) {
+        const int b = i / W, e = rp[b] + (i - b * W);
+        const bool in = e < rp[b + 1];
+        ev[i] = in ? gv[e] : make_double2(0.0, 0.0);
+        ec[i] = in ? gc[e] : 0;
+      }
+      Kpar[x] = EllS{smem_addr(ev), smem_addr(ec)};
+    }
     kd[0] = reinterpret_cast<c64*>(nxt);
     kd[1] = kd[0] + NB;
     for (int i = tid; i < NB; i += kFwdThreads17) {
-      kd[0][i] = p.csr.diag[m0 * NB + i];
-      kd[1][i] = p.csr.diag[m1 * NB + i];
+      kd[0][i] = p.csr.diag[mm[0] * NB + i];
+      kd[1][i] = p.csr.diag[mm[1] * NB + i];
     }
-    kdiag[0] = (p.csr.diag_mask >> m0) & 1;
-    kdiag[1] = (p.csr.diag_mask >> m1) & 1;
+    kdiag[0] = (p.csr.diag_mask >> mm[0]) & 1;
+    kdiag[1] = (p.csr.diag_mask >> mm[1]) & 1;
   }
   Rare17* rare = rare_all + t;
   __syncthreads();                          // the only CTA barrier: from here every warp runs on its own
@@ -233,7 +258,7 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
         S[1] = cmul(n2, S[1]);
         S[2] = cmul(n2, S[2]);
       } else {
-        sparse_left17(R, S, Kpar[par], mat_s, l8);
+        sparse_left17(R, S, Kpar[par], W, mat_s, l8);
       }
     }
     if (s == N - 1) {
@@ -302,7 +327,9 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
         if (l8 == 0) mat_t[16 * NB + 16] = S[2];
       }
     } else {
-      sparse_right_dagger17(R, S, Kpar[parn], mat_s, mat_t, tmp_s, l8);   // ytilde_s = g_s K_{s+1}^dagger
+      // ytilde_s = g_s K_{s+1}^dagger
+      if (W == 2) sparse_right_dagger17<2>(R, S, Kpar[parn], W, mat_s, mat_t, tmp_s, l8);
+      else sparse_right_dagger17<0>(R, S, Kpar[parn], W, mat_s, mat_t, tmp_s, l8);
     }
     __syncwarp();
     store_row17(h + l8 * kHistLd17, R[0]);
@@ -322,16 +349,16 @@ cudaError_t launch_block_fwd17(const SweepLaunch& p, cudaStream_t s) {
   const long long first = p.cta_begin > p.n_eq_cta ? p.cta_begin : p.n_eq_cta;
   const long long n = p.cta_begin + p.n_cta - first;
   if (n <= 0) return cudaSuccess;
-  const size_t smem = fwd17_smem(p.csr.nnz_cap);
+  const size_t smem = fwd17_smem(p.csr.row_nnz_max);
   cudaError_t e = cudaFuncSetAttribute(block_fwd17_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   block_fwd17_kernel<<<(unsigned)n, kFwdThreads17, smem, s>>>(p, first);
   return cudaGetLastError();
 }
 
-int block_fwd17_ctas_per_sm(int nnz_cap) {
+int block_fwd17_ctas_per_sm(int row_nnz_max) {
   int nb = 0;
-  const size_t smem = fwd17_smem(nnz_cap);
+  const size_t smem = fwd17_smem(row_nnz_max);
   if (cudaFuncSetAttribute(block_fwd17_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return 0;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, block_fwd17_kernel, kFwdThreads17, smem) != cudaSuccess)

@@ -37,6 +37,7 @@ struct BlockPath {
   double2* csr_diag;
   int diag_mask;
   int nnz_cap;
+  int row_nnz_max;
   double2* lead_mats;
   double2* table;
   double2* hist;
@@ -160,6 +161,10 @@ negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, c
     }
     rowptr[m * (n + 1) + n] = e;
   }
+  bp->row_nnz_max = 1;
+  for (int m = 0; m < 4; ++m)
+    for (int r = 0; r < n; ++r)
+      bp->row_nnz_max = std::max(bp->row_nnz_max, rowptr[m * (n + 1) + r + 1] - rowptr[m * (n + 1) + r]);
   // lead 0 (left, rings -1, -2, ...): V0 = H_{-1,-2} = E^dagger, V1 = H_{-2,-3} = O^dagger,
   //   Sigma_L = tau^dagger g tau with tau = H_{-1,0} = O          -> (L, R) = (O^dagger, O)
   // lead 1 (right, rings N, N+1, ...): V0 = H_{N,N+1}, V1 = H_{N+1,N+2},
@@ -231,7 +236,7 @@ negf_status block_path_create(const negf_config* cfg, const double2* z_eq_dev, c
   int dev = 0, sms = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  bp->ctas_per_sm = blk::block_sweep_ctas_per_sm(n, nnz_cap);
+  bp->ctas_per_sm = blk::block_sweep_ctas_per_sm(n, nnz_cap, bp->row_nnz_max);
   if (bp->ctas_per_sm < 1) {
     cudaGetLastError();
     set_error("negf_create: the block sweep kernel does not fit on this device (n = %d, nnz = %d)", n, nnz_cap);
@@ -302,6 +307,7 @@ blk::SweepLaunch sweep_launch(const BlockPath* bp, const double* U_dev, double* 
   p.probe_ring = probe_ring; p.probe = probe;
   p.csr.rowptr = bp->csr_rowptr; p.csr.col = bp->csr_col; p.csr.val = bp->csr_val;
   p.csr.nnz_cap = bp->nnz_cap;
+  p.csr.row_nnz_max = bp->row_nnz_max;
   p.csr.diag = bp->csr_diag; p.csr.diag_mask = bp->diag_mask;
   p.cta_begin = 0;
   p.n_cta = 0;

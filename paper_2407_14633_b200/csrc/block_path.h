@@ -41,6 +41,7 @@ struct CsrSet {
   const int* col;        // [4][nnz_cap]
   const double2* val;    // [4][nnz_cap]
   int nnz_cap;           // max nnz over the four
+  int row_nnz_max;       // max nnz of a row over the four (width of the padded row tables of block_fwd17.cu)
   const double2* diag;   // [4][nb] diagonal entries of the four matrices
   int diag_mask;         // bit m set: matrix m is diagonal (its products stay in registers)
 };
@@ -96,7 +97,7 @@ constexpr int kHistRec17 = 17 * kHistLd17;   // history elements per task and ri
 constexpr int kBackThreads17 = 256;   // 8 warps = the 8 tasks of one block_fwd17 CTA
 cudaError_t launch_block_back17(const SweepLaunch& p, cudaStream_t s);
 cudaError_t launch_block_fwd17(const SweepLaunch& p, cudaStream_t s);    // block_fwd17.cu
-int block_fwd17_ctas_per_sm(int nnz_cap);
+int block_fwd17_ctas_per_sm(int row_nnz_max);
 // Contour combine over the pairs of contour CTAs [cta_begin, cta_begin + 2 n_pairs) of a finished
 // sweep launch whose first CTA was launch_cta_begin.
 cudaError_t launch_block_combine(int nb, const SweepLaunch& p, long long pair_cta_begin, int n_pairs,
@@ -107,7 +108,7 @@ int block_tasks_per_cta_real(int nb);   // real-axis CTAs (n = 17: block_fwd17.c
 int block_threads(int nb);
 long long block_step_elems(int nb);   // history elements per ring step per CTA
 size_t block_sweep_smem(int nb, int nnz_cap);
-int block_sweep_ctas_per_sm(int nb, int nnz_cap);
+int block_sweep_ctas_per_sm(int nb, int nnz_cap, int row_nnz_max);
 bool block_size_supported(int nb);
 
 }  // namespace blk

@@ -604,9 +604,9 @@ size_t block_sweep_smem(int nb, int nnz_cap) {
     default: return 0;
   }
 }
-int block_sweep_ctas_per_sm(int nb, int nnz_cap) {
+int block_sweep_ctas_per_sm(int nb, int nnz_cap, int row_nnz_max) {
   if (nb == 17) {                      // both forward kernels must fit; the real-axis one carries the load
-    const int a = ctas_per_sm_t<17>(nnz_cap), b = block_fwd17_ctas_per_sm(nnz_cap);
+    const int a = ctas_per_sm_t<17>(nnz_cap), b = block_fwd17_ctas_per_sm(row_nnz_max);
     return a < 1 ? a : b;
   }
   switch (nb) {
