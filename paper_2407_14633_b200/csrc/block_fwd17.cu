@@ -180,17 +180,19 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
 #define NEGF_TAB_LAST (p.table + tab_off + (dir ? 0 : 2 * MAT))
 
   // couplings of this direction, by parity of the bond: [0] even bond, [1] odd bond (as in block_sweep.cu)
+  // Nothing here is an array indexed by the parity: such arrays live in local memory, and a local load per
+  // ring showed up as 10 % long-scoreboard stalls.  The two tables are a fixed stride apart instead.
   const int W = p.csr.row_nnz_max;
-  EllS Kpar[2];
-  c64* kd[2];
-  bool kdiag[2];
+  const unsigned ell_stride = (unsigned)(((size_t)NB * W * (sizeof(c64) + sizeof(int)) + 15) / 16 * 16);
+  const unsigned ell0 = smem_addr(nxt);            // table x: values at ell0 + x * ell_stride, then the columns
+  c64* kd0 = reinterpret_cast<c64*>(nxt + 2 * ell_stride);   // diagonals: kd0 + x * NB
+  int diag_bits = 0;                               // bit x: coupling x is a diagonal matrix
   {
     const int mm[2] = {dir ? CSR_E : CSR_EDAG, dir ? CSR_O : CSR_ODAG};
 #pragma unroll
     for (int x = 0; x < 2; ++x) {
-      c64* ev = reinterpret_cast<c64*>(nxt);
+      c64* ev = reinterpret_cast<c64*>(nxt + x * ell_stride);
       int* ec = reinterpret_cast<int*>(ev + NB * W);
-      nxt = reinterpret_cast<char*>((reinterpret_cast<uintptr_t>(ec + NB * W) + 15) & ~uintptr_t(15));
       const int* rp = p.csr.rowptr + mm[x] * (NB + 1);
       const int* gc = p.csr.col + (size_t)mm[x] * p.csr.nnz_cap;
       const c64* gv = p.csr.val + (size_t)mm[x] * p.csr.nnz_cap;
@@ -200,17 +202,11 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
         ev[i] = in ? gv[e] : make_double2(0.0, 0.0);
         ec[i] = in ? gc[e] : 0;
       }
-      Kpar[x] = EllS{smem_addr(ev), smem_addr(ec)};
+      for (int i = tid; i < NB; i += kFwdThreads17) kd0[x * NB + i] = p.csr.diag[mm[x] * NB + i];
+      diag_bits |= ((p.csr.diag_mask >> mm[x]) & 1) << x;
     }
-    kd[0] = reinterpret_cast<c64*>(nxt);
-    kd[1] = kd[0] + NB;
-    for (int i = tid; i < NB; i += kFwdThreads17) {
-      kd[0][i] = p.csr.diag[mm[0] * NB + i];
-      kd[1][i] = p.csr.diag[mm[1] * NB + i];
-    }
-    kdiag[0] = (p.csr.diag_mask >> mm[0]) & 1;
-    kdiag[1] = (p.csr.diag_mask >> mm[1]) & 1;
   }
+  auto ell = [&](int x) { return EllS{ell0 + x * ell_stride, ell0 + x * ell_stride + (unsigned)(NB * W * sizeof(c64))}; };
   Rare17* rare = rare_all + t;
   __syncthreads();                          // the only CTA barrier: from here every warp runs on its own
 
@@ -218,16 +214,13 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
   const unsigned mat_s = smem_addr(mat_t);
   const unsigned tmp_s = smem_addr(tmp_all + (size_t)tid * NB);
   c64* hrec = p.hist + (size_t)(gid - p.cta_begin) * N * STEP + (size_t)t * kHistRec17;   // + s * STEP
-  const double* Uc = p.U + (size_t)c * N;
-  double u_next = Uc[dir ? N - 1 : 0];      // potential of the next ring, loaded one ring ahead
 
   // Loop invariant at the top of step s > 0: R, S = the lane's share of ytilde_{s-1}; if the coupling
   // entering step s is not diagonal, ytilde_{s-1} is also in the task's shared-memory matrix.
   c64 R[2][NB], S[3];
   for (int s = 0; s < N; ++s) {
     const int i = dir ? N - 1 - s : s;
-    const double zu = z.x - u_next;
-    if (s < N - 1) u_next = Uc[dir ? i - 1 : i + 1];
+    const double u_i = p.U[(size_t)c * N + i];     // used after the product below: the load has time
     if (s == 0) {
       const c64* tab = NEGF_TAB_FIRST;
 #pragma unroll
@@ -244,8 +237,8 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
     } else {
       const int par = dir ? (i & 1) : ((i - 1) & 1);
       // d := -K_s ytilde_{s-1}
-      if (kdiag[par]) {
-        const c64* kdp = kd[par];
+      if ((diag_bits >> par) & 1) {
+        const c64* kdp = kd0 + par * NB;
         const c64 k0 = kdp[l8], k1 = kdp[l8 + 8], k2 = kdp[16];
         const c64 n0 = make_double2(-k0.x, -k0.y), n1 = make_double2(-k1.x, -k1.y);
         const c64 n2 = make_double2(-k2.x, -k2.y);
@@ -258,7 +251,7 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
         S[1] = cmul(n2, S[1]);
         S[2] = cmul(n2, S[2]);
       } else {
-        sparse_left17(R, S, Kpar[par], W, mat_s, l8);
+        sparse_left17(R, S, ell(par), W, mat_s, l8);
       }
     }
     if (s == N - 1) {
@@ -276,6 +269,7 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
       S[1].x -= v1.x; S[1].y -= v1.y;
       S[2].x -= v2.x; S[2].y -= v2.y;
     }
+    const double zu = z.x - u_i;
 #pragma unroll
     for (int b = 0; b < 8; ++b)
       if (b == l8) {
@@ -307,12 +301,12 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
     if (s < N - 1) {
       const int inext = dir ? i - 1 : i + 1;
       parn = dir ? (inext & 1) : ((inext - 1) & 1);
-      next_diag = kdiag[parn];
+      next_diag = (diag_bits >> parn) & 1;
     }
     c64* h = hrec + (size_t)s * STEP;
     if (s == N - 1 || next_diag) {
       if (s < N - 1) {                       // ytilde_ab = g_ab conj(K_bb); last ring: G_(k,k) itself
-        const c64* kdn = kd[parn];
+        const c64* kdn = kd0 + parn * NB;
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
           const c64 kb = cconj(kdn[b]);
@@ -328,8 +322,8 @@ __global__ void __launch_bounds__(kFwdThreads17, 4) block_fwd17_kernel(const Swe
       }
     } else {
       // ytilde_s = g_s K_{s+1}^dagger
-      if (W == 2) sparse_right_dagger17<2>(R, S, Kpar[parn], W, mat_s, mat_t, tmp_s, l8);
-      else sparse_right_dagger17<0>(R, S, Kpar[parn], W, mat_s, mat_t, tmp_s, l8);
+      if (W == 2) sparse_right_dagger17<2>(R, S, ell(parn), W, mat_s, mat_t, tmp_s, l8);
+      else sparse_right_dagger17<0>(R, S, ell(parn), W, mat_s, mat_t, tmp_s, l8);
     }
     __syncwarp();
     store_row17(h + l8 * kHistLd17, R[0]);
