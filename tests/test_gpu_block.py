@@ -96,6 +96,23 @@ def test_forced_column_search_matches():
         assert_parity(T, T_ref, f"{w.name} forced-search T(E)")
 
 
+@pytest.mark.parametrize("theta", [0.05, 0.25, 0.6])
+def test_threshold_pivoting_paths_of_the_n17_forward_kernel(theta):
+    """block_fwd17.cu at n = 17 has three pivoting paths: diagonal candidates, the in-register column search
+    (candidate rejected by the row-norm test) and the shared-memory slow path (corner d rejected as first
+    pivot; pivot_theta = 1e150 above sends every ring there).  Large but finite thresholds reject a good share
+    of the diagonal candidates while the corner still passes for part of the warps, so the column search, the
+    permutation through shared memory and mixed warps (tasks on different paths) all run; results must match
+    the dense definition.  Real-space tube and random sparse non-symmetric complex couplings."""
+    wl3 = wlmod.make_config(3, N=12, K_neq=37, K_eq=5)
+    wl17 = _random_block_workload(17, N=9, K_neq=21, K_eq=3, seed=178, sparse=True)
+    for w in (wl3, wl17):
+        n_ref, T_ref = od.charge_and_transmission(w)
+        n, T = _gpu_run(w, pivot_theta=theta)
+        assert_parity(n, n_ref, f"{w.name} theta={theta} charge")
+        assert_parity(T, T_ref, f"{w.name} theta={theta} T(E)")
+
+
 def test_integrand_probe_generic_block_sizes():
     """SURVEY 8(f)-2 on the SIMT way back of the generic block sizes (n != 17): integrand at a probe ring
     and its peak against the dense definition, random non-symmetric complex blocks."""
