@@ -29,6 +29,7 @@
 #include <math_constants.h>
 
 #include "block_ops.cuh"
+#include "cgemm17.cuh"
 #include "block_path.h"
 #include "negf_internal.h"
 
@@ -166,19 +167,50 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
     }
     __syncthreads();
     const int rb = (1 - h) * NB;   // half 0 works on g11 / g10, half 1 on g00 / g01
-    c64 ar[NB], pq[NB], res[NB];
-    row_from<NB>(ar, mine + a * NB);
-    gemm_row_ld<NB, N2>(pq, ar, Gt + rb * N2 + rb);          // Y g11   | X g00
-    gemm_row<NB>(res, pq, other);                            // Y g11 X | X g00 Y
-    if (!frozen) {
-#pragma unroll
-      for (int b = 0; b < NB; ++b) {
-        eh[b].x += res[b].x; eh[b].y += res[b].y;
-        es[b].x += res[b].x; es[b].y += res[b].y;            // only meaningful for half 1
+    c64 res[NB];
+    if constexpr (NB == 17) {
+      // The eight n x n products of the pass on the tensor cores (cgemm17.cuh), one warp per product, in place
+      // in the blocks of Gt: first the four left factors X, Y, then the four right factors.  (As rows of
+      // register products they were a quarter of the kernel's stall samples and 200 registers of live rows.)
+      const int warp = tid >> 5, lane = tid & 31;
+      c64* xy = reinterpret_cast<c64*>(nxt);
+#pragma unroll 1
+      for (int stage = 0; stage < 2; ++stage) {
+#pragma unroll 1
+        for (int item = warp; item < 4 * G2::TPC; item += G2::NWARPS) {
+          const int tt = item >> 2, w = item & 3;            // w = 0: Y g11 (X), 1: X g00 (Y), 2: Y g10 (Y), 3: X g01 (X)
+          c64* Xt = xy + (size_t)tt * 2 * MATN;
+          c64* Yt = Xt + MATN;
+          c64* blk = sm.mat + (size_t)tt * G2::MAT + (w == 0 ? NB * N2 + NB : w == 1 ? 0 : w == 2 ? NB * N2 : NB);
+          if (stage == 0) cgemm17_warp((w & 1) ? Xt : Yt, NB, blk, N2, blk, N2, lane);
+          else cgemm17_warp(blk, N2, (w == 0 || w == 3) ? Xt : Yt, NB, blk, N2, lane);
+        }
+        __syncthreads();
       }
+      row_from<NB>(res, Gt + (rb + a) * N2 + rb);            // Y g11 X | X g00 Y
+      if (!frozen) {
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+          eh[b].x += res[b].x; eh[b].y += res[b].y;
+          es[b].x += res[b].x; es[b].y += res[b].y;
+        }
+      }
+      row_from<NB>(res, Gt + (rb + a) * N2 + (NB - rb));     // Y g10 Y | X g01 X
+    } else {
+      c64 ar[NB], pq[NB];
+      row_from<NB>(ar, mine + a * NB);
+      gemm_row_ld<NB, N2>(pq, ar, Gt + rb * N2 + rb);          // Y g11   | X g00
+      gemm_row<NB>(res, pq, other);                            // Y g11 X | X g00 Y
+      if (!frozen) {
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+          eh[b].x += res[b].x; eh[b].y += res[b].y;
+          es[b].x += res[b].x; es[b].y += res[b].y;            // only meaningful for half 1
+        }
+      }
+      gemm_row_ld<NB, N2>(pq, ar, Gt + rb * N2 + (NB - rb));   // Y g10   | X g01
+      gemm_row<NB>(res, pq, mine);                             // Y g10 Y | X g01 X
     }
-    gemm_row_ld<NB, N2>(pq, ar, Gt + rb * N2 + (NB - rb));   // Y g10   | X g01
-    gemm_row<NB>(res, pq, mine);                             // Y g10 Y | X g01 X
     if (frozen) {
 #pragma unroll
       for (int b = 0; b < NB; ++b) res[b] = make_double2(0.0, 0.0);
