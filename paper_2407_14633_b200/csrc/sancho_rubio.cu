@@ -316,49 +316,106 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
     row_to<NB>((h == 0 ? Pb : Qb) + a * NB, pqrow, live);
     __syncthreads();
     bool pdone = false;
-    for (int it = 0; it < kDoublingMax; ++it) {
-      c64 w[NB];
-      if (h == 0) {
-        gemm_row<NB>(w, dlt, Qb);                            // D Q
-        row_to<NB>(Tb + a * NB, w, live);
-      } else {
-        gemm_row<NB>(w, pqrow, Qb);                          // Q^2
-#pragma unroll
-        for (int b = 0; b < NB; ++b) pqrow[b] = pdone ? make_double2(0.0, 0.0) : w[b];
-      }
+    if constexpr (NB == 17) {
+      // the doubling sum on the tensor cores (cgemm17.cuh): P, Q, T = D Q and D are the four n x n blocks of Gt
+      c64* Db = Gt + 3 * MATN;
+      row_to<NB>(Db + a * NB, dlt, live0);
       __syncthreads();
-      double rowmax = 0.0;
-      c64 p2[NB];
-      if (h == 0) {
-        gemm_row<NB>(w, pqrow, Tb);                          // P D Q
-        if (!pdone) {
-#pragma unroll
-          for (int b = 0; b < NB; ++b) { dlt[b].x += w[b].x; dlt[b].y += w[b].y; }
+      const int warp = tid >> 5, lane = tid & 31;
+      for (int it = 0; it < kDoublingMax; ++it) {
+#pragma unroll 1
+        for (int tt = warp; tt < G2::TPC; tt += G2::NWARPS) {          // T = D Q
+          c64* g = sm.mat + (size_t)tt * G2::MAT;
+          cgemm17_warp(g + 3 * MATN, NB, g + MATN, NB, g + 2 * MATN, NB, lane);
         }
-      } else {
-        c64 ar[NB];
-        row_from<NB>(ar, Pb + a * NB);
-        gemm_row<NB>(p2, ar, Pb);                            // P^2 (computed by half 1 to balance the work)
-        if (pdone) {
-#pragma unroll
-          for (int b = 0; b < NB; ++b) p2[b] = make_double2(0.0, 0.0);
+        __syncthreads();
+#pragma unroll 1
+        for (int item = warp; item < 2 * G2::TPC; item += G2::NWARPS) {
+          c64* g = sm.mat + (size_t)(item >> 1) * G2::MAT;
+          if (item & 1) {
+            cgemm17_warp(g + MATN, NB, g + MATN, NB, g + MATN, NB, lane);        // Q <- Q^2
+          } else {
+            cgemm17_warp(g, NB, g + 2 * MATN, NB, g + 2 * MATN, NB, lane);      // T <- P D Q
+            cgemm17_warp(g, NB, g, NB, g, NB, lane);                            // P <- P^2
+          }
         }
-        rowmax = fmax(row_absmax<NB>(p2), row_absmax<NB>(pqrow));
-      }
-      if (live) sm.mag[t * N2 + r] = rowmax;
-      __syncthreads();                                       // reads of Pb, Qb, Tb done
-      if (h == 1) {
-        row_to<NB>(Pb + a * NB, p2, live);
-        row_to<NB>(Qb + a * NB, pqrow, live);
-      }
-      double tmax = 0.0;
+        __syncthreads();
+        double rowmax = 0.0;
+        if (h == 0) {
+          if (!pdone) {
+            c64 w[NB];
+            row_from<NB>(w, Tb + a * NB);
 #pragma unroll
-      for (int i = 0; i < N2; ++i) tmax = fmax(tmax, sm.mag[t * N2 + i]);
-      if (tmax < 1e-4) pdone = true;                         // |P_j| |Q_j| < 1e-8: series summed
-      if (!(tmax < 1e6)) { pdone = true; div_now = true; }   // growing powers: spectral radius > 1
-      const bool all_done = __syncthreads_and(pdone || !live);
-      if (h == 0) row_from<NB>(pqrow, Pb + a * NB);
-      if (all_done) break;
+            for (int b = 0; b < NB; ++b) { dlt[b].x += w[b].x; dlt[b].y += w[b].y; }
+            row_to<NB>(Db + a * NB, dlt, live);
+          }
+        } else {
+          c64 w[NB];
+          row_from<NB>(w, Pb + a * NB);
+          rowmax = row_absmax<NB>(w);
+          row_from<NB>(w, Qb + a * NB);
+          rowmax = fmax(rowmax, row_absmax<NB>(w));
+          if (pdone) rowmax = 0.0;
+        }
+        if (live) sm.mag[t * N2 + r] = rowmax;
+        __syncthreads();
+        double tmax = 0.0;
+#pragma unroll
+        for (int i = 0; i < N2; ++i) tmax = fmax(tmax, sm.mag[t * N2 + i]);
+        const bool was_done = pdone;
+        if (tmax < 1e-4) pdone = true;                         // |P_j| |Q_j| < 1e-8: series summed
+        if (!(tmax < 1e6)) { pdone = true; div_now = true; }   // growing powers: spectral radius > 1
+        if (pdone && !was_done && h == 1 && live) {            // a finished task adds nothing any more
+#pragma unroll
+          for (int b = 0; b < NB; ++b) Pb[a * NB + b] = Qb[a * NB + b] = make_double2(0.0, 0.0);
+        }
+        if (__syncthreads_and(pdone || !live)) break;
+      }
+    } else {
+        for (int it = 0; it < kDoublingMax; ++it) {
+        c64 w[NB];
+        if (h == 0) {
+          gemm_row<NB>(w, dlt, Qb);                            // D Q
+          row_to<NB>(Tb + a * NB, w, live);
+        } else {
+          gemm_row<NB>(w, pqrow, Qb);                          // Q^2
+  #pragma unroll
+          for (int b = 0; b < NB; ++b) pqrow[b] = pdone ? make_double2(0.0, 0.0) : w[b];
+        }
+        __syncthreads();
+        double rowmax = 0.0;
+        c64 p2[NB];
+        if (h == 0) {
+          gemm_row<NB>(w, pqrow, Tb);                          // P D Q
+          if (!pdone) {
+  #pragma unroll
+            for (int b = 0; b < NB; ++b) { dlt[b].x += w[b].x; dlt[b].y += w[b].y; }
+          }
+        } else {
+          c64 ar[NB];
+          row_from<NB>(ar, Pb + a * NB);
+          gemm_row<NB>(p2, ar, Pb);                            // P^2 (computed by half 1 to balance the work)
+          if (pdone) {
+  #pragma unroll
+            for (int b = 0; b < NB; ++b) p2[b] = make_double2(0.0, 0.0);
+          }
+          rowmax = fmax(row_absmax<NB>(p2), row_absmax<NB>(pqrow));
+        }
+        if (live) sm.mag[t * N2 + r] = rowmax;
+        __syncthreads();                                       // reads of Pb, Qb, Tb done
+        if (h == 1) {
+          row_to<NB>(Pb + a * NB, p2, live);
+          row_to<NB>(Qb + a * NB, pqrow, live);
+        }
+        double tmax = 0.0;
+  #pragma unroll
+        for (int i = 0; i < N2; ++i) tmax = fmax(tmax, sm.mag[t * N2 + i]);
+        if (tmax < 1e-4) pdone = true;                         // |P_j| |Q_j| < 1e-8: series summed
+        if (!(tmax < 1e6)) { pdone = true; div_now = true; }   // growing powers: spectral radius > 1
+        const bool all_done = __syncthreads_and(pdone || !live);
+        if (h == 0) row_from<NB>(pqrow, Pb + a * NB);
+        if (all_done) break;
+      }
     }
     // X <- X + D, written where the next pass (or the code below) expects the 00 block
     __syncthreads();
