@@ -29,6 +29,7 @@
 #include <math_constants.h>
 
 #include "block_ops.cuh"
+#include "block_ops34.cuh"
 #include "cgemm17.cuh"
 #include "block_path.h"
 #include "negf_internal.h"
@@ -97,6 +98,25 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
   c64* Yb = Xb + MATN;                                             // n x n
   c64* mine = h == 0 ? Yb : Xb;    // half 0 carries Y (-> eps_00, new Y), half 1 carries X
   c64* other = h == 0 ? Xb : Yb;
+  // n = 17: the 34 x 34 inversions run one warp per task (block_ops34.cuh), on the matrix in shared memory
+  int* perm34 = reinterpret_cast<int*>(reinterpret_cast<c64*>(nxt) + (size_t)G2::TPC * 2 * MATN);
+  // the thread's row m of the 2n x 2n matrix -> the inverse in Gt; the caller places __syncthreads() after
+  // fast: the decimation passes, whose result the Newton polish corrects; the surface Green's function and the
+  // polish itself keep gj_invert (pivots in row order): the warp version, which takes rows 32, 33 first, left
+  // T(E) of config 4 off by 3.6e-10 at one energy when it was used there too
+  auto invert_to_Gt = [&](c64 (&m)[N2], bool fast) {
+    if (NB == 17 && fast) {
+      __syncthreads();                                             // nobody reads the old Gt any more
+      row_to<N2>(Gt + r * N2, m, live);
+      __syncthreads();
+      const int warp = tid >> 5;
+      if (warp < G2::TPC)
+        invert34_w32(sm.mat + (size_t)warp * G2::MAT, perm34 + warp * 32, p.theta2, tid & 31);
+    } else {
+      const bool permuted = gj_invert<N2>(m, sm, t, r, live, p.theta2);
+      store_inverse<N2>(m, Gt, sm, t, r, live, permuted);
+    }
+  };
 
   const int K_all = p.K_eq + p.K_neq;
   const long long n_task = p.task_end;
@@ -162,8 +182,7 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
     {
       c64 m[N2];
       build_row(m, eh, zd);
-      const bool permuted = gj_invert<N2>(m, sm, t, r, live, p.theta2);
-      store_inverse<N2>(m, Gt, sm, t, r, live, permuted);
+      invert_to_Gt(m, true);
     }
     __syncthreads();
     const int rb = (1 - h) * NB;   // half 0 works on g11 / g10, half 1 on g00 / g01
@@ -247,8 +266,7 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
 #pragma unroll
     for (int b = 0; b < NB; ++b) ed[b] = h == 0 ? make_double2(b == a ? U : 0.0, 0.0) : es[b];
     build_row(m, ed, zd);
-    const bool permuted = gj_invert<N2>(m, sm, t, r, live, p.theta2);
-    store_inverse<N2>(m, Gt, sm, t, r, live, permuted);
+    invert_to_Gt(m, false);
 #pragma unroll
     for (int b = 0; b < NB; ++b)
       if (live) mine[a * NB + b] = my_init[b];               // Xb = V1, Yb = V1^+ again
@@ -275,8 +293,7 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
           if (b == a) ed[b].x += U;
       }
       build_row(m, ed, z);
-      const bool permuted = gj_invert<N2>(m, sm, t, r, live, p.theta2);
-      store_inverse<N2>(m, Gt, sm, t, r, live, permuted);    // Gt = G(X)
+      invert_to_Gt(m, false);
     }
     __syncthreads();
     c64 dlt[NB];                   // half 0: residual row, then the Newton correction
@@ -511,7 +528,8 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
 
 template <int NB>
 static size_t sr_smem_t() {
-  return Smem<2 * NB>::bytes(1) + sizeof(c64) * (size_t)Geo<2 * NB>::TPC * 2 * NB * NB + 32;
+  return Smem<2 * NB>::bytes(1) + sizeof(c64) * (size_t)Geo<2 * NB>::TPC * 2 * NB * NB +
+         sizeof(int) * 32 * Geo<2 * NB>::TPC + 32;
 }
 
 template <int NB>
