@@ -96,7 +96,11 @@ typedef struct {
                                  accepted without a search when |a_kk| >= theta * ||row k of the matrix handed
                                  in||_2; otherwise the task searches the whole column (partial pivoting).
                                  0 = default (1e-4); a huge value (1e150) forces the search at every
-                                 elimination step (test hook).                                             */
+                                 elimination step (test hook).  block = 17: the warp-resident inversions
+                                 (real-axis forward sweep, decimation passes of the lead self-energies) apply
+                                 the same test to the corner row(s) they eliminate first and fall back to
+                                 plain partial pivoting in shared memory when it fails, so 1e150 sends every
+                                 such inversion through that fallback.                                       */
 } negf_config;
 
 /* Create a handle: validates, copies the config, allocates workspace.  `cuda_stream` is a
