@@ -153,7 +153,7 @@ static __device__ __noinline__ void invert34_w32(c64* m, int* perm, double theta
   perm[lane] = lane;
   bool used = false, any_search = false;
   c64 dinv = make_double2(1.0, 0.0);
-#pragma unroll 1
+#pragma unroll 2
   for (int k = 0; k < 32; ++k) {
     const double mm = cabs2(R[0]);
     const int cand_ok = (!used && (mm >= thr) && (mm > 0.0)) ? 1 : 0;
