@@ -12,7 +12,7 @@
 // Because H01 has a single non-zero n x n block, the decimation matrices keep that shape for ever,
 //     a = |1> X <0|,  b = |0> Y <1|,   X = V1, Y = V1^+ initially,
 // and with g = (z - eps)^-1 (2n x 2n, four n x n blocks g00 g01 g10 g11) one pass is
-//     eps_11 += X g00 Y;  eps_s,11 += X g00 Y;  eps_00 += Y g11 X;  X <- X g01 X;  Y <- Y g10 Y,
+//     eps_11 += X g00 Y;  eps_s,11 += X g00 Y (= eps_11);  eps_00 += Y g11 X;  X <- X g01 X;  Y <- Y g10 Y,
 // the off-diagonal blocks of eps staying V0, V0^+.  So the only 2n x 2n operation is the inversion;
 // the eight products are n x n.  Loop until max|X_ij|, |Y_ij| < sr_tol, plus two more passes.
 //
@@ -165,12 +165,12 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
   for (int attempt = 0; attempt < 2; ++attempt) {
   const c64 zd = diverged ? make_double2(z.x, z.y + p.shift) : z;
   bool div_now = false;
-  c64 eh[NB];          // row a of eps_hh
-  c64 es[NB];          // row a of eps_s,11 (half 1; half 0 keeps eps_s,00 = U I)
+  // row a of eps_hh.  The surface block eps_s,11 receives the same increments X g00 Y as eps_11 and eps_s,00
+  // stays U I, so eps_s needs no storage of its own.
+  c64 eh[NB];
 #pragma unroll
   for (int b = 0; b < NB; ++b) {
     eh[b] = make_double2(b == a ? U : 0.0, 0.0);
-    es[b] = eh[b];
     if (live) mine[a * NB + b] = my_init[b];
   }
   int remaining = -1;  // -1: criterion not met yet; >= 0: passes still to do after it was met
@@ -211,7 +211,6 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
           eh[b].x += res[b].x; eh[b].y += res[b].y;
-          es[b].x += res[b].x; es[b].y += res[b].y;
         }
       }
       row_from<NB>(res, Gt + (rb + a) * N2 + (NB - rb));     // Y g10 Y | X g01 X
@@ -224,7 +223,6 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
           eh[b].x += res[b].x; eh[b].y += res[b].y;
-          es[b].x += res[b].x; es[b].y += res[b].y;            // only meaningful for half 1
         }
       }
       gemm_row_ld<NB, N2>(pq, ar, Gt + rb * N2 + (NB - rb));   // Y g10   | X g01
@@ -264,7 +262,7 @@ __global__ void __launch_bounds__(Geo<2 * NB>::THREADS, 1) sancho_rubio_kernel(c
   {
     c64 m[N2], ed[NB];
 #pragma unroll
-    for (int b = 0; b < NB; ++b) ed[b] = h == 0 ? make_double2(b == a ? U : 0.0, 0.0) : es[b];
+    for (int b = 0; b < NB; ++b) ed[b] = h == 0 ? make_double2(b == a ? U : 0.0, 0.0) : eh[b];
     build_row(m, ed, zd);
     invert_to_Gt(m, false);
 #pragma unroll
